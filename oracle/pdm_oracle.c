@@ -1,0 +1,174 @@
+/*
+ * pdm_oracle.c -- TEST INFRASTRUCTURE ONLY.  Plain, slow, FP64 CPU statement of the hot path
+ * of explicit f-x poststack depth migration, written from the paper
+ * (arXiv 1912.05529, /root/reference/PAPER.md) for checking the CUDA library against.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may build, load or call this file.  It shares no code, header, table or helper with the
+ * CUDA path (paper_1912_05529_b200/csrc) and must never be reachable from the product path.
+ *
+ * What it computes (citations are PAPER.md lines; R# are the readings listed in DESIGN.md):
+ *
+ *   Eq. (1), PAPER.md:45      u(x_i, w_r, z_{k+1}) = sum_{n=-(N-1)/2}^{(N-1)/2} h[n] u(x_{i-n}, w_r, z_k)
+ *   Alg. 1,  PAPER.md:59-70   for each depth level { for each frequency { for each space {
+ *                               look-up table (pre-designed 1-D FIR filters); extrapolate } }
+ *                               depth row = sum over frequencies }              (nesting: R1)
+ *   PAPER.md:83               the filter ("cutoff") depends on frequency and velocity and may
+ *                             differ from point to point: it is looked up per OUTPUT point (R8)
+ *
+ *   O1  q32[z][x] = (float)( (double)dz / ((double)v32[z][x] * du) )          (R3: one rounding)
+ *   O2  for each w (independent):
+ *   O3      P[x] = (complex double) P0[w][x]
+ *   O4      for z = 0 .. nz-1:                                               (sequential)
+ *   O5        for x = 0 .. nx-1:
+ *   O6          idx = clamp( lrintf( w32 * q32[z][x] ), 0, ntab-1 )          (R3: FLOAT product,
+ *                                                                             round half to even)
+ *   O7          acc = sum_{k=-L..L, 0 <= x-k < nx}  table[idx][L+k] * P[x-k] (Eq. 1; R5 zero edges;
+ *                                                                             R11 orientation)
+ *   O8          Pnew[x] = acc
+ *   O9        swap(P, Pnew)
+ *   O10       img_w[z][x] = Re P[x]      row z = field AFTER step z, depth (z+1) dz   (R6, R7)
+ *   O11 image[z][x] = sum_w img_w[z][x]  in FP64, fixed order                 (R10)
+ *
+ * No symmetric folding, no tiling, no blocking: the full 2L+1 row is applied literally.
+ * Parallelism: OpenMP over w only (independent lines); per-thread FP64 image accumulators
+ * are summed in thread-id order, and each thread walks its w in increasing order, so the
+ * result is deterministic for a fixed thread count.
+ *
+ * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): P1 delta table = identity, P2 brute
+ * force on tiny grids, P3 spectral identity, P4 exact phase shift in constant velocity,
+ * P5 point-diffractor focusing, P7 superposition, P8 w-additivity/permutation, P9 mirror,
+ * P10 energy non-growth, P11 shift invariance, P12 index rule.  Parity unpinned by anything
+ * external: the choices R5/R6/R7 (boundary, row<->depth, velocity row) and the absolute
+ * amplitude scale R10 -- fixed by DESIGN.md only.
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef struct { float re, im; } oracle_c64;
+
+#define ORACLE_OK 0
+#define ORACLE_ERR_ARG -1
+#define ORACLE_ERR_NOMEM -2
+
+int pdm_oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* O1 + O6 exposed on their own so pin P12 can test the index rule directly. */
+int pdm_oracle_index(float omega, float velocity, double dz, double du, int ntab)
+{
+    float q32 = (float)(dz / ((double)velocity * du));
+    float prod = omega * q32;                 /* float x float -> float, no FMA involved */
+    long j = lrintf(prod);                    /* default rounding mode: half to even     */
+    if (j < 0) j = 0;
+    if (j > ntab - 1) j = ntab - 1;
+    return (int)j;
+}
+
+/*
+ * All pointers are HOST pointers.  image_out is double [nz][nx] (O12: never rounded down).
+ * If wavefield_out != NULL it receives the final field P(z = nz dz) as interleaved
+ * complex double [nw][nx] (used by pins P3/P4/P10 which look at the field, not the image).
+ * omega_subset: if nsub > 0, only lines omega_index[0..nsub) are migrated (bench sampling, P8).
+ */
+int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
+                       const float *omega, const float *velocity,
+                       const oracle_c64 *table, int ntab, int ntaps, double du,
+                       const oracle_c64 *P0,
+                       const int *omega_index, int nsub,
+                       double *image_out, double *wavefield_out)
+{
+    if (nx <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0 ||
+        !(du > 0.0) || !omega || !velocity || !table || !P0 || !image_out)
+        return ORACLE_ERR_ARG;
+    const int L = (ntaps - 1) / 2;
+    const int nlines = nsub > 0 ? nsub : nw;
+    const size_t plane = (size_t)nz * (size_t)nx;
+
+    /* O1 */
+    float *q32 = (float *)malloc(plane * sizeof(float));
+    if (!q32) return ORACLE_ERR_NOMEM;
+    for (size_t i = 0; i < plane; ++i)
+        q32[i] = (float)(dz / ((double)velocity[i] * du));
+
+    int nthreads = pdm_oracle_num_threads();
+    if (nthreads > nlines) nthreads = nlines;
+    double *acc = (double *)calloc((size_t)nthreads * plane, sizeof(double));
+    if (!acc) { free(q32); return ORACLE_ERR_NOMEM; }
+    int failed = 0;
+
+#pragma omp parallel num_threads(nthreads)
+    {
+#ifdef _OPENMP
+        const int tid = omp_get_thread_num();
+#else
+        const int tid = 0;
+#endif
+        double *img = acc + (size_t)tid * plane;
+        double *P = (double *)malloc(sizeof(double) * 2 * (size_t)nx);
+        double *Pn = (double *)malloc(sizeof(double) * 2 * (size_t)nx);
+        if (!P || !Pn) {
+#pragma omp atomic write
+            failed = 1;
+        } else {
+#pragma omp for schedule(static)
+            for (int il = 0; il < nlines; ++il) {                       /* O2 */
+                const int iw = nsub > 0 ? omega_index[il] : il;
+                const float w32 = omega[iw];
+                for (int x = 0; x < nx; ++x) {                          /* O3 */
+                    P[2 * x] = (double)P0[(size_t)iw * nx + x].re;
+                    P[2 * x + 1] = (double)P0[(size_t)iw * nx + x].im;
+                }
+                for (int z = 0; z < nz; ++z) {                          /* O4 */
+                    const float *qrow = q32 + (size_t)z * nx;
+                    for (int x = 0; x < nx; ++x) {                      /* O5 */
+                        float prod = w32 * qrow[x];                     /* O6 */
+                        long j = lrintf(prod);
+                        if (j < 0) j = 0;
+                        if (j > ntab - 1) j = ntab - 1;
+                        const oracle_c64 *row = table + (size_t)j * ntaps;
+                        double ar = 0.0, ai = 0.0;
+                        for (int k = -L; k <= L; ++k) {                 /* O7 */
+                            int xs = x - k;
+                            if (xs < 0 || xs >= nx) continue;
+                            double wr = (double)row[L + k].re, wi = (double)row[L + k].im;
+                            double pr = P[2 * xs], pi = P[2 * xs + 1];
+                            ar += wr * pr - wi * pi;
+                            ai += wr * pi + wi * pr;
+                        }
+                        Pn[2 * x] = ar;                                 /* O8 */
+                        Pn[2 * x + 1] = ai;
+                    }
+                    { double *t = P; P = Pn; Pn = t; }                  /* O9 */
+                    double *irow = img + (size_t)z * nx;                /* O10 (+ O11 partial) */
+                    for (int x = 0; x < nx; ++x) irow[x] += P[2 * x];
+                }
+                if (wavefield_out)
+                    memcpy(wavefield_out + 2 * (size_t)il * nx, P, sizeof(double) * 2 * (size_t)nx);
+            }
+        }
+        free(P);
+        free(Pn);
+    }
+
+    if (!failed) {                                                      /* O11: fixed thread order */
+        for (size_t i = 0; i < plane; ++i) {
+            double s = 0.0;
+            for (int t = 0; t < nthreads; ++t) s += acc[(size_t)t * plane + i];
+            image_out[i] = s;
+        }
+    }
+    free(acc);
+    free(q32);
+    return failed ? ORACLE_ERR_NOMEM : ORACLE_OK;
+}
