@@ -1,0 +1,157 @@
+/*
+ * pdm.h -- C ABI of libpdm: the hot path of explicit f-x poststack depth migration
+ * (arXiv 1912.05529; citations are /root/reference/PAPER.md lines; R# = readings in DESIGN.md).
+ *
+ * What the library computes (and nothing else):
+ *
+ *   Eq. (1), PAPER.md:45      P(z+dz, w, x) = sum_{k=-L..L} W_k(u(x,z,w)) * P(z, w, x-k)
+ *   PAPER.md:65, :83          the 2L+1-tap extrapolator W(u) is LOOKED UP in a pre-designed table,
+ *                             per output point, by u = w*dz/v(x,z)                 (R3, R8)
+ *   PAPER.md:59-70, :85       marched over every depth level; after each level the depth row is
+ *                             image[z][x] = sum_w Re P(z+dz, w, x)                 (R1, R6, R10)
+ *
+ *   index rule (R3)           q32[z][x] = (float)((double)dz / ((double)v32[z][x] * tab_du))
+ *                             idx = clamp(rint_half_even(fl32(w32 * q32)), 0, ntab-1)
+ *   edges (R5)                samples with x-k outside [0,nx) contribute zero
+ *   rows (R6, R7)             step iz uses velocity row iz; image row iz = field AFTER step iz
+ *
+ * Every entry point returns PDM_OK (0) or a negative pdm_status; nothing throws or aborts
+ * across the ABI.  All sizes are element counts; all arrays are dense row-major.
+ * "HOST" / "DEVICE" says where a pointer must point.  There is no CPU fallback: without a
+ * compute-capability-10.x device pdm_create fails with PDM_ERR_UNSUPPORTED.
+ */
+#ifndef PDM_H
+#define PDM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct pdm_plan pdm_plan;            /* opaque; owned by the library                        */
+typedef struct { float re, im; } pdm_c64;    /* == torch.complex64 / numpy.complex64 / cuFloatComplex */
+
+typedef enum {
+    PDM_OK = 0,
+    PDM_ERR_INVALID_ARG = -1,      /* NULL pointer, dim <= 0, ntaps even or < 1, tab_du <= 0,
+                                      non-finite or <= 0 velocity / omega, unknown flag bits       */
+    PDM_ERR_TABLE_RANGE = -2,      /* some rint(w*q) > ntab-1 (kernels still clamp defensively)    */
+    PDM_ERR_TABLE_ASYMMETRIC = -3, /* table[j][L+k] != table[j][L-k] bitwise: the kernels fold the
+                                      symmetric taps (W_k == W_-k, north_star) and would silently
+                                      compute something else                                       */
+    PDM_ERR_UNSUPPORTED = -4,      /* not a CC 10.x device; forced path impossible for this nx;
+                                      ntaps above PDM_MAX_TAPS                                     */
+    PDM_ERR_NOMEM = -5,            /* host or device allocation failed                             */
+    PDM_ERR_CUDA = -6              /* a CUDA call failed; pdm_info.last_cuda_error has the code    */
+} pdm_status;
+
+#define PDM_MAX_TAPS 129           /* L <= 64 */
+
+/* flags word of pdm_create: bits 0-3 choose the kernel form, the rest are tuning/debug knobs.     */
+#define PDM_PATH_AUTO    0u  /* SMEM marching if a line (ping-pong) fits one CTA, else x-tiled      */
+#define PDM_PATH_SMEM    1u  /* main form: one CTA keeps a frequency's x-line in shared memory and   */
+                             /* marches all nz depth steps in place (north_star)       */
+#define PDM_PATH_TILED   2u  /* x-tiled per-depth-step kernel with +-L halos, planes ping-pong in HBM*/
+#define PDM_PATH_NAIVE   3u  /* scaffold: one thread per (w,x) sample, one launch per depth level --  */
+                             /* the paper's own mapping, kept only as a cross-check    */
+#define PDM_PATH_CLUSTER 4u  /* line split over a thread-block cluster with DSMEM halos              */
+#define PDM_PATH_MASK    0xFu
+#define PDM_TAPS_AUTO    (0u << 4)  /* where the kernels read filter rows from                      */
+#define PDM_TAPS_GLOBAL  (1u << 4)  /* always from the L2/L1-cached global half-table               */
+#define PDM_TAPS_SLICE   (2u << 4)  /* per-frequency contiguous row slice staged in shared memory   */
+#define PDM_TAPS_COMPACT (3u << 4)  /* per-frequency list of the rows actually used, staged in SMEM */
+#define PDM_TAPS_MASK    (0x3u << 4)
+#define PDM_FORCE_GENERAL (1u << 6) /* debug: never take the uniform-index fast path                */
+#define PDM_NO_BALANCE   (1u << 7)  /* debug: whole lines per CTA (no depth-split load balancing)   */
+#define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto)                   */
+#define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto)   */
+#define PDM_TILE_SHIFT    20        /* bits 20-27: x-tile size / 256 samples for PDM_PATH_TILED     */
+#define PDM_FLAGS_VALID  0x0FFFFFFFu
+
+typedef struct {
+    int    path;                 /* PDM_PATH_* actually chosen                                      */
+    int    taps_mode;            /* PDM_TAPS_* >> 4 actually chosen                                 */
+    int    nx, nz, nw, ntab, ntaps;
+    int    grid_ctas;            /* CTAs of the dominant kernel                                     */
+    int    threads_per_cta;
+    int    ctas_per_sm;
+    int    smem_bytes;           /* dynamic shared memory per CTA of the dominant kernel            */
+    int    launches_per_migrate; /* kernels one pdm_migrate call enqueues                           */
+    int    sm_count;
+    int    last_cuda_error;      /* cudaError_t of the last failing CUDA call (0 if none)           */
+    double samples;              /* nx*nz*nw: extrapolated (z,w,x) points per migrate               */
+    double counted_flops;        /* 8*(2L+1)*samples (metric definition, BASELINE.json north_star)  */
+    double executed_lane_ops;    /* (6L+4)*samples FP32 lane operations with symmetric folding      */
+    double workspace_bytes;      /* device memory the plan owns                                     */
+} pdm_info;
+
+/*
+ * pdm_create -- validate, pre-digest and upload everything that does not depend on the data.
+ *   out       HOST  receives the plan; *out = NULL on failure.
+ *   nx,nz,nw  lateral samples, depth steps, frequencies.
+ *   dx,dz     metres.  dx is metadata only (it enters through the filter design, R9).
+ *   omega     HOST  float[nw], rad/s, any order, finite, > 0.
+ *   velocity  HOST  float[nz][nx], m/s, finite, > 0: the MIGRATION velocity; the library computes
+ *             exactly u = w*dz/velocity (the caller passes v/2 for two-way-time data, R2).
+ *   table     HOST  pdm_c64[ntab][ntaps]; table[j][L+k] = W_k(u_j), u_j = j*tab_du, k = -L..L (R11);
+ *             must be bitwise symmetric in k.
+ *   flags     PDM_PATH_* | PDM_TAPS_* | tuning bits.
+ * The caller may free all its arrays on return.  The plan is bound to the CUDA device that is
+ * current at the call.  Not thread-safe per plan; different plans are independent.
+ */
+int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, float dz,
+               const float *omega, const float *velocity,
+               const pdm_c64 *table, int ntab, int ntaps, double tab_du,
+               unsigned flags);
+
+/*
+ * pdm_migrate -- the timed call: march P0 through all nz depth levels and image it.
+ *   P0_dev     DEVICE pdm_c64[nw][nx]  f-x section at z = 0, read-only, not modified.
+ *   image_dev  DEVICE float[nz][nx]    overwritten with sum_w Re P after every step.
+ *   cuda_stream  cudaStream_t (0 = legacy default stream).
+ * Asynchronous on the stream; performs no allocation, no host synchronisation and no host<->device
+ * copy (CUDA-graph capturable); bit-identical images on repeated calls (fixed summation order, no
+ * float atomics).  One migrate in flight per plan (the workspace is per plan).
+ * Errors: PDM_ERR_INVALID_ARG (NULL), PDM_ERR_CUDA (launch failure, wrong current device).
+ */
+int pdm_migrate(pdm_plan *plan, const pdm_c64 *P0_dev, float *image_dev, void *cuda_stream);
+
+/*
+ * pdm_migrate_host -- same operation with HOST buffers (the end-to-end call): copies P0 to the
+ * device, runs pdm_migrate, copies the image back and synchronises the stream before returning.
+ *   P0_host    HOST pdm_c64[nw][nx] (pinned memory makes the copies asynchronous and faster).
+ *   image_host HOST float[nz][nx].
+ * Uses staging buffers owned by the plan (allocated on first use: PDM_ERR_NOMEM possible).
+ */
+int pdm_migrate_host(pdm_plan *plan, const pdm_c64 *P0_host, float *image_host, void *cuda_stream);
+
+/* pdm_destroy -- free all device and host state of the plan.  NULL is allowed. */
+int pdm_destroy(pdm_plan *plan);
+
+/* pdm_get_info -- fill *out (HOST) with the plan's launch configuration and work counts. */
+int pdm_get_info(const pdm_plan *plan, pdm_info *out);
+
+/* pdm_strerror -- static string for a pdm_status (never NULL). */
+const char *pdm_strerror(int code);
+
+/*
+ * pdm_debug_table_index -- DEVICE evaluation of the index rule R3 (pin P12 on the GPU side):
+ *   idx_dev[i] = clamp(rint(fl32(omega_dev[i] * q)), 0, ntab-1), q = (float)(dz/(velocity_dev[i]*tab_du))
+ * with q formed on the HOST side of the library exactly as pdm_create does (so velocity is HOST).
+ *   omega HOST float[n], velocity HOST float[n], idx_out HOST int[n].  Synchronous.
+ */
+int pdm_debug_table_index(const float *omega, const float *velocity, int n,
+                          double dz, double tab_du, int ntab, int *idx_out);
+
+/*
+ * pdm_fp32_peak -- FP32-FMA throughput microbenchmark (independent FFMA chains on every SM),
+ * the denominator of the "% of FP32 FMA peak" metric.  Runs `iters` chain iterations on
+ * `cuda_stream` and returns the best of `repeats` timings.
+ *   packed       0 = scalar FFMA, 1 = packed fma.rn.f32x2 (FFMA2)
+ *   tflops_out   HOST double: achieved 1e12 flop/s (2 flops per FMA lane-op)
+ */
+int pdm_fp32_peak(int packed, int iters, int repeats, void *cuda_stream, double *tflops_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PDM_H */

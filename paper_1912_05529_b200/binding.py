@@ -1,0 +1,234 @@
+"""ctypes binding of libpdm.so: same names and argument order as include/pdm.h.
+
+Marshalling only.  If the shared library is missing this module raises -- there is no Python,
+PyTorch or CPU implementation of the path to fall back to.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libpdm.so")
+_lib = None
+
+PDM_OK = 0
+PDM_ERR_INVALID_ARG = -1
+PDM_ERR_TABLE_RANGE = -2
+PDM_ERR_TABLE_ASYMMETRIC = -3
+PDM_ERR_UNSUPPORTED = -4
+PDM_ERR_NOMEM = -5
+PDM_ERR_CUDA = -6
+
+PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER = 0, 1, 2, 3, 4
+PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
+PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TILE_SHIFT = 8, 16, 20
+
+EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
+                    "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak")
+
+
+class PdmInfo(ctypes.Structure):
+    _fields_ = [("path", ctypes.c_int), ("taps_mode", ctypes.c_int),
+                ("nx", ctypes.c_int), ("nz", ctypes.c_int), ("nw", ctypes.c_int),
+                ("ntab", ctypes.c_int), ("ntaps", ctypes.c_int),
+                ("grid_ctas", ctypes.c_int), ("threads_per_cta", ctypes.c_int),
+                ("ctas_per_sm", ctypes.c_int), ("smem_bytes", ctypes.c_int),
+                ("launches_per_migrate", ctypes.c_int), ("sm_count", ctypes.c_int),
+                ("last_cuda_error", ctypes.c_int),
+                ("samples", ctypes.c_double), ("counted_flops", ctypes.c_double),
+                ("executed_lane_ops", ctypes.c_double), ("workspace_bytes", ctypes.c_double)]
+
+    def as_dict(self) -> dict:
+        return {name: getattr(self, name) for name, _ in self._fields_}
+
+
+class PdmError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = int(code)
+        super().__init__(f"{where}: {pdm_strerror(code)} ({code})")
+
+
+def load_library(path: str | None = None):
+    """dlopen libpdm.so (built in-tree by paper_1912_05529_b200.build.build_lib). Raises if absent."""
+    global _lib
+    if _lib is not None and path is None:
+        return _lib
+    path = path or _LIB_PATH
+    if not os.path.exists(path):
+        raise RuntimeError(f"{path} is missing: build it with __graft_entry__.build() "
+                           "(nvcc, sm_100a). There is no fallback implementation.")
+    lib = ctypes.CDLL(path)
+    vp, ci, cf, cd, cu = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_double, ctypes.c_uint
+    lib.pdm_create.restype = ci
+    lib.pdm_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cf, cf, vp, vp, vp, ci, ci, cd, cu]
+    lib.pdm_migrate.restype = ci
+    lib.pdm_migrate.argtypes = [vp, vp, vp, vp]
+    lib.pdm_migrate_host.restype = ci
+    lib.pdm_migrate_host.argtypes = [vp, vp, vp, vp]
+    lib.pdm_destroy.restype = ci
+    lib.pdm_destroy.argtypes = [vp]
+    lib.pdm_get_info.restype = ci
+    lib.pdm_get_info.argtypes = [vp, ctypes.POINTER(PdmInfo)]
+    lib.pdm_strerror.restype = ctypes.c_char_p
+    lib.pdm_strerror.argtypes = [ci]
+    lib.pdm_debug_table_index.restype = ci
+    lib.pdm_debug_table_index.argtypes = [vp, vp, ci, cd, cd, ci, vp]
+    lib.pdm_fp32_peak.restype = ci
+    lib.pdm_fp32_peak.argtypes = [ci, ci, ci, vp, ctypes.POINTER(cd)]
+    _lib = lib
+    return lib
+
+
+_STRERROR_LOCAL = {0: "ok", -1: "invalid argument", -2: "table range", -3: "table asymmetric",
+                   -4: "unsupported", -5: "out of memory", -6: "CUDA call failed"}
+
+
+def pdm_strerror(code: int) -> str:
+    try:
+        return load_library().pdm_strerror(int(code)).decode()
+    except RuntimeError:
+        return _STRERROR_LOCAL.get(int(code), "unknown")
+
+
+# ------------------------------------------------------------------ raw calls (names of pdm.h)
+def pdm_create(nx, nz, nw, dx, dz, omega, velocity, table, tab_du, flags=0):
+    """-> (status, plan handle or None).  omega/velocity/table are HOST numpy arrays."""
+    lib = load_library()
+    omega = np.ascontiguousarray(omega, dtype=np.float32)
+    velocity = np.ascontiguousarray(velocity, dtype=np.float32)
+    table = np.ascontiguousarray(table, dtype=np.complex64)
+    if omega.shape != (nw,) or velocity.shape != (nz, nx) or table.ndim != 2:
+        return PDM_ERR_INVALID_ARG, None
+    ntab, ntaps = table.shape
+    handle = ctypes.c_void_p()
+    rc = lib.pdm_create(ctypes.byref(handle), int(nx), int(nz), int(nw), float(dx), float(dz),
+                        omega.ctypes.data, velocity.ctypes.data, table.ctypes.data,
+                        int(ntab), int(ntaps), float(tab_du), int(flags))
+    return rc, (handle if rc == PDM_OK else None)
+
+
+def pdm_migrate(plan, P0_dev_ptr: int, image_dev_ptr: int, cuda_stream: int = 0) -> int:
+    return load_library().pdm_migrate(plan, ctypes.c_void_p(P0_dev_ptr), ctypes.c_void_p(image_dev_ptr),
+                                      ctypes.c_void_p(cuda_stream))
+
+
+def pdm_migrate_host(plan, P0_host_ptr: int, image_host_ptr: int, cuda_stream: int = 0) -> int:
+    return load_library().pdm_migrate_host(plan, ctypes.c_void_p(P0_host_ptr),
+                                           ctypes.c_void_p(image_host_ptr), ctypes.c_void_p(cuda_stream))
+
+
+def pdm_destroy(plan) -> int:
+    return load_library().pdm_destroy(plan)
+
+
+def pdm_get_info(plan) -> PdmInfo:
+    info = PdmInfo()
+    rc = load_library().pdm_get_info(plan, ctypes.byref(info))
+    if rc != PDM_OK:
+        raise PdmError(rc, "pdm_get_info")
+    return info
+
+
+def pdm_debug_table_index(omega, velocity, dz, tab_du, ntab) -> np.ndarray:
+    omega = np.ascontiguousarray(omega, dtype=np.float32)
+    velocity = np.ascontiguousarray(velocity, dtype=np.float32)
+    out = np.empty(omega.size, dtype=np.int32)
+    rc = load_library().pdm_debug_table_index(omega.ctypes.data, velocity.ctypes.data, int(omega.size),
+                                              float(dz), float(tab_du), int(ntab), out.ctypes.data)
+    if rc != PDM_OK:
+        raise PdmError(rc, "pdm_debug_table_index")
+    return out
+
+
+def pdm_fp32_peak(packed: bool = True, iters: int = 20000, repeats: int = 5, cuda_stream: int = 0) -> float:
+    val = ctypes.c_double()
+    rc = load_library().pdm_fp32_peak(int(bool(packed)), int(iters), int(repeats),
+                                      ctypes.c_void_p(cuda_stream), ctypes.byref(val))
+    if rc != PDM_OK:
+        raise PdmError(rc, "pdm_fp32_peak")
+    return float(val.value)
+
+
+# ------------------------------------------------------------------ convenience wrapper
+class Plan:
+    """Owns a pdm_plan.  `cfg` is a workload dict in the pdm_inputs layout (or pass the fields)."""
+
+    def __init__(self, nx, nz, nw, dx, dz, omega, velocity, table, tab_du, flags=0):
+        rc, handle = pdm_create(nx, nz, nw, dx, dz, omega, velocity, table, tab_du, flags)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_create")
+        self._h = handle
+        self.nx, self.nz, self.nw = int(nx), int(nz), int(nw)
+
+    @classmethod
+    def from_config(cls, cfg: dict, flags: int = 0) -> "Plan":
+        return cls(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"],
+                   cfg["velocity"], cfg["table"], cfg["du"], flags)
+
+    @property
+    def info(self) -> dict:
+        return pdm_get_info(self._h).as_dict()
+
+    def migrate(self, P0, image=None, stream=None):
+        """P0: torch.complex64 CUDA tensor [nw, nx] -> image torch.float32 CUDA [nz, nx] (async)."""
+        import torch
+        if not (P0.is_cuda and P0.dtype == torch.complex64 and P0.is_contiguous()
+                and tuple(P0.shape) == (self.nw, self.nx)):
+            raise ValueError("P0 must be a contiguous CUDA complex64 tensor [nw, nx]")
+        if image is None:
+            image = torch.empty((self.nz, self.nx), dtype=torch.float32, device=P0.device)
+        elif not (image.is_cuda and image.dtype == torch.float32 and image.is_contiguous()
+                  and tuple(image.shape) == (self.nz, self.nx)):
+            raise ValueError("image must be a contiguous CUDA float32 tensor [nz, nx]")
+        st = (stream or torch.cuda.current_stream(P0.device)).cuda_stream
+        rc = pdm_migrate(self._h, P0.data_ptr(), image.data_ptr(), st)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_migrate")
+        return image
+
+    def migrate_host(self, P0_host, image_host=None, stream=None):
+        """End-to-end call: HOST complex64 [nw, nx] (numpy or pinned torch) -> HOST float32 [nz, nx]."""
+        import torch
+        if isinstance(P0_host, np.ndarray):
+            P0_host = np.ascontiguousarray(P0_host, dtype=np.complex64)
+            src_ptr, shape = P0_host.ctypes.data, P0_host.shape
+        else:
+            if P0_host.is_cuda or P0_host.dtype != torch.complex64 or not P0_host.is_contiguous():
+                raise ValueError("P0_host must be a contiguous host complex64 tensor")
+            src_ptr, shape = P0_host.data_ptr(), tuple(P0_host.shape)
+        if tuple(shape) != (self.nw, self.nx):
+            raise ValueError("P0_host must be [nw, nx]")
+        if image_host is None:
+            image_host = np.empty((self.nz, self.nx), dtype=np.float32)
+        if isinstance(image_host, np.ndarray):
+            if image_host.dtype != np.float32 or not image_host.flags.c_contiguous:
+                raise ValueError("image_host must be contiguous float32")
+            dst_ptr = image_host.ctypes.data
+        else:
+            dst_ptr = image_host.data_ptr()
+        st = (stream.cuda_stream if stream is not None
+              else torch.cuda.current_stream().cuda_stream)
+        rc = pdm_migrate_host(self._h, src_ptr, dst_ptr, st)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_migrate_host")
+        return image_host
+
+    def close(self):
+        if self._h is not None:
+            pdm_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,248 @@
+// kern_march.cuh -- PDM_PATH_SMEM, the main form (BASELINE.json north_star; "block
+// level synchronization" instead of kernel exit):
+//   one CTA keeps one frequency's x-line in shared memory (ping-pong) and marches ALL nz depth
+//   steps without the wavefield ever returning to HBM.  Per depth step:
+//     A1  j = clamp(rint(w*q[z][x]))                  (R3; q rows come from L2, one pass ahead)
+//     A2  taps W_0..W_L of row j                      (half table; rows this w can touch are staged
+//                                                      in shared memory, else read through L1)
+//     A3  P'(x) = W_0 P(x) + sum_k W_k (P(x-k)+P(x+k)) (Eq. (1) PAPER.md:45 folded with W_k == W_-k)
+//     A4  __syncthreads, swap buffers
+//     A5  partial[cta][z][x] (+)= Re P'(x)            (fixed order; pdm_reduce_partials sums CTAs)
+//
+// Register tiling: a thread owns R consecutive outputs ("group").  For tap k it needs the two
+// R-wide windows P[x0-k .. x0+R-1-k] and P[x0+k .. x0+R-1+k]; going from k to k+1 each window
+// slides by one sample, so with the k loop fully unrolled the windows live in 2R register pairs
+// and every wavefield sample is read from shared memory once per thread (as 16-byte pairs).
+// Arithmetic is packed FP32 (FFMA2/FADD2): per (k, output) one FADD2 (re,im of the folded sum)
+// and two FFMA2 with the scalar-broadcast operand form (acc_a += Wr*S, acc_b += Wi*S); the
+// complex result is (a.x - b.y, a.y + b.x).
+//
+// Shared-memory line layout: groups of R samples followed by 2 pad samples, HG all-zero halo
+// groups on both sides (R5: zero outside [0,nx), so no edge branches).  Lane stride is then
+// (R+2)*8 B, which makes the 16-byte window loads / stores of a quarter-warp bank-conflict free.
+#pragma once
+#include "pdm_common.cuh"
+
+#define PDM_MARCH_MAX_THREADS 384
+
+struct pdm_march_params {
+    const float2 *P0;        // [nw][nx]
+    float        *partial;   // [grid][nz][pstride]
+    const float  *q;         // [nz][qstride]
+    const float  *omega;     // [nw]
+    const float4 *half;      // [ntab][half16]
+    const int    *rowoff;    // [nw+1]
+    const int    *rows;      // row lists
+    int nx, nz, nw, ntab;
+    int qstride, pstride, half16;
+    int ngroups, passes, slots, map_len;
+};
+
+__host__ __device__ constexpr int pdm_floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
+__host__ __device__ constexpr int pdm_mod(int a, int b) { return a - pdm_floordiv(a, b) * b; }
+// slot offset (in float2) of sample x0+m relative to the slot of x0 (x0 = first sample of a group)
+template <int R> __host__ __device__ constexpr int pdm_soff(int m) { return m + 2 * pdm_floordiv(m, R); }
+template <int L, int R> __host__ __device__ constexpr int pdm_halo_groups() { return (L + 1 + R - 1) / R; }
+
+__device__ __forceinline__ float2 f4lo(float4 v) { return make_float2(v.x, v.y); }
+__device__ __forceinline__ float2 f4hi(float4 v) { return make_float2(v.z, v.w); }
+
+// One group of R outputs.  `base` = &line[slot(x0)];  tbase + toff[r] = first float4 of the half
+// row of output r (all equal when UNIFORM, in which case only toff[0] is read).  tbase is passed
+// separately from the offsets so that after inlining the compiler still knows its address space.
+template <int L, int R, bool UNIFORM>
+__device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
+                                              const float4 *__restrict__ tbase,
+                                              const int (&toff)[R], float2 (&out)[R])
+{
+    float2 wl[R], wr[R], acc_a[R], acc_b[R];
+    float4 tw[UNIFORM ? 1 : R];
+#pragma unroll
+    for (int i = 0; i < R / 2; ++i) {
+        const float4 v = *reinterpret_cast<const float4 *>(base + 2 * i);
+        wl[2 * i] = f4lo(v); wl[2 * i + 1] = f4hi(v);
+        wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
+    }
+#pragma unroll
+    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r]];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {                       // centre tap W_0
+        const float4 t = tw[UNIFORM ? 0 : r];
+        acc_a[r] = pk_mul_s(t.x, wl[r]);
+        acc_b[r] = pk_mul_s(t.y, wl[r]);
+    }
+    float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
+#pragma unroll
+    for (int k = 1; k <= L; ++k) {
+        if (k & 1) {                                    // two new samples per side serve k and k+1
+            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(-k - 1));
+            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(R + k - 1));
+            wl[pdm_mod(-k, R)] = f4hi(lv);
+            wr[pdm_mod(k - 1, R)] = f4lo(rv);
+        } else {
+            wl[pdm_mod(-k, R)] = f4lo(lv);
+            wr[pdm_mod(k - 1, R)] = f4hi(rv);
+#pragma unroll
+            for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r] + k / 2];
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            const float wre = (k & 1) ? t.z : t.x, wim = (k & 1) ? t.w : t.y;
+            const float2 s = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
+            acc_a[r] = pk_fma_s(wre, s, acc_a[r]);
+            acc_b[r] = pk_fma_s(wim, s, acc_b[r]);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
+}
+
+template <int L, int R, bool TAPS_SMEM>
+__global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(const pdm_march_params p)
+{
+    static_assert(R % 2 == 0 && R >= 2, "R must be even");
+    constexpr int HG = pdm_halo_groups<L, R>();
+    constexpr int GS = R + 2;
+    extern __shared__ __align__(16) unsigned char pdm_smem[];
+    float2 *buf_a = reinterpret_cast<float2 *>(pdm_smem);
+    float2 *buf_b = buf_a + p.slots;
+    unsigned short *map = reinterpret_cast<unsigned short *>(buf_b + p.slots);
+    float4 *slice = reinterpret_cast<float4 *>(map + p.map_len);
+
+    const int tid = threadIdx.x, T = blockDim.x;
+    const int ntab_m1 = p.ntab - 1;
+    for (int i = tid; i < p.slots; i += T)              // 2*slots float2 = slots float4
+        reinterpret_cast<float4 *>(buf_a)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+
+    float *const my_partial = p.partial + (size_t)blockIdx.x * p.nz * p.pstride;
+    bool first = true;
+
+    for (int line = blockIdx.x; line < p.nw; line += gridDim.x) {
+        __syncthreads();                                 // previous line (and the zero fill) done
+        const float w = p.omega[line];
+        if (TAPS_SMEM) {                                 // A2 staging: rows this omega can touch
+            const int r0 = p.rowoff[line], nrows = p.rowoff[line + 1] - r0;
+            for (int i = tid; i < nrows; i += T) map[p.rows[r0 + i]] = (unsigned short)i;
+            const int n4 = nrows * p.half16;
+            for (int e = tid; e < n4; e += T) {
+                const int s = e / p.half16, c = e - s * p.half16;
+                slice[e] = p.half[(size_t)p.rows[r0 + s] * p.half16 + c];
+            }
+        }
+        {                                                // P(z=0) = P0[line]
+            const float2 *src = p.P0 + (size_t)line * p.nx;
+            for (int x = tid; x < p.nx; x += T) {
+                const int g = x / R;
+                buf_a[(HG + g) * GS + (x - g * R)] = src[x];
+            }
+        }
+        __syncthreads();
+
+        float2 *cur = buf_a, *nxt = buf_b;
+        float qn[R];
+        {
+            const int g0 = min(tid, p.ngroups - 1);
+            const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)g0 * R);
+#pragma unroll
+            for (int i = 0; i < R / 4; ++i) {
+                const float4 v = __ldg(qp + i);
+                qn[4 * i] = v.x; qn[4 * i + 1] = v.y; qn[4 * i + 2] = v.z; qn[4 * i + 3] = v.w;
+            }
+        }
+        for (int z = 0; z < p.nz; ++z) {
+            for (int pass = 0; pass < p.passes; ++pass) {
+                const int g_raw = pass * T + tid;
+                // whole warp beyond the line: nothing to do in this pass (warp-uniform)
+                const bool warp_active = (pass * T + (tid & ~31)) < p.ngroups;
+                float qc[R];
+#pragma unroll
+                for (int r = 0; r < R; ++r) qc[r] = qn[r];
+                {                                        // A1 prefetch: q of the next (z, pass)
+                    int pz = z, pp = pass + 1;
+                    if (pp == p.passes) { pp = 0; ++pz; }
+                    if (pz < p.nz) {
+                        const int gn = min(pp * T + tid, p.ngroups - 1);
+                        const float4 *qp = reinterpret_cast<const float4 *>(
+                            p.q + (size_t)pz * p.qstride + (size_t)gn * R);
+#pragma unroll
+                        for (int i = 0; i < R / 4; ++i) {
+                            const float4 v = __ldg(qp + i);
+                            qn[4 * i] = v.x; qn[4 * i + 1] = v.y; qn[4 * i + 2] = v.z; qn[4 * i + 3] = v.w;
+                        }
+                    }
+                }
+                if (!warp_active) continue;
+                const bool active = g_raw < p.ngroups;
+                const int g = active ? g_raw : p.ngroups - 1;
+
+                float4 *prow = reinterpret_cast<float4 *>(my_partial + (size_t)z * p.pstride + (size_t)g * R);
+                float4 pold[R / 4];
+                if (!first) {                            // A5: old partial row, consumed at the end
+#pragma unroll
+                    for (int i = 0; i < R / 4; ++i) pold[i] = __ldcs(prow + i);
+                } else {
+#pragma unroll
+                    for (int i = 0; i < R / 4; ++i) pold[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                }
+
+                int j[R];
+                bool uni = true;
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    j[r] = pdm_index(w, qc[r], ntab_m1);
+                    uni = uni && (j[r] == j[0]);
+                }
+                int toff[R];
+                const float4 *tbase = TAPS_SMEM ? slice : p.half;
+                const float2 *base = cur + (HG + g) * GS;
+                float2 out[R];
+                if (__all_sync(0xffffffffu, uni)) {
+                    toff[0] = (TAPS_SMEM ? (int)map[j[0]] : j[0]) * p.half16;
+#pragma unroll
+                    for (int r = 1; r < R; ++r) toff[r] = toff[0];
+                    pdm_fir_group<L, R, true>(base, tbase, toff, out);
+                } else {
+#pragma unroll
+                    for (int r = 0; r < R; ++r) toff[r] = (TAPS_SMEM ? (int)map[j[r]] : j[r]) * p.half16;
+                    pdm_fir_group<L, R, false>(base, tbase, toff, out);
+                }
+                if (active) {
+                    const int x0 = g * R;
+                    float2 *dst = nxt + (HG + g) * GS;
+#pragma unroll
+                    for (int i = 0; i < R / 2; ++i) {    // samples beyond nx stay zero (R5)
+                        float2 a = out[2 * i], b = out[2 * i + 1];
+                        if (x0 + 2 * i >= p.nx) a = make_float2(0.f, 0.f);
+                        if (x0 + 2 * i + 1 >= p.nx) b = make_float2(0.f, 0.f);
+                        *reinterpret_cast<float4 *>(dst + 2 * i) = make_float4(a.x, a.y, b.x, b.y);
+                    }
+#pragma unroll
+                    for (int i = 0; i < R / 4; ++i) {
+                        float4 v = pold[i];
+                        v.x += out[4 * i].x; v.y += out[4 * i + 1].x;
+                        v.z += out[4 * i + 2].x; v.w += out[4 * i + 3].x;
+                        __stcs(prow + i, v);
+                    }
+                }
+            }
+            __syncthreads();                             // A4: step z complete for the whole line
+            float2 *t = cur; cur = nxt; nxt = t;
+        }
+        first = false;
+    }
+}
+
+// A5, second half: image[z][x] = sum over CTAs (fixed order) of their partial images.
+__global__ void pdm_reduce_partials(const float *__restrict__ partial, float *__restrict__ image,
+                                    int nparts, int nz, int nx, int pstride)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x;
+    const int z = blockIdx.y;
+    if (x >= nx) return;
+    const size_t plane = (size_t)nz * pstride;
+    const float *src = partial + (size_t)z * pstride + x;
+    float s = 0.f;
+    for (int c = 0; c < nparts; ++c) s += __ldcs(src + (size_t)c * plane);
+    image[(size_t)z * nx + x] = s;
+}

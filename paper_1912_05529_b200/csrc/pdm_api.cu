@@ -1,0 +1,497 @@
+// pdm_api.cu -- host side of libpdm: the C ABI declared in include/pdm.h.
+// Everything data-independent is validated, pre-digested and uploaded in pdm_create; pdm_migrate
+// only enqueues kernels on the caller's stream.  There is no CPU fallback anywhere in this file:
+// without a compute-capability-10.x device pdm_create fails with PDM_ERR_UNSUPPORTED.
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "pdm_common.cuh"
+#include "kern_naive.cuh"
+#include "kern_peak.cuh"
+#include "kern_march.cuh"
+#include "kern_tiled.cuh"
+
+#define PDM_CUDA(plan, call)                                                        \
+    do {                                                                            \
+        cudaError_t e_ = (call);                                                    \
+        if (e_ != cudaSuccess) {                                                    \
+            if (plan) (plan)->last_cuda_error = (int)e_;                            \
+            return e_ == cudaErrorMemoryAllocation ? PDM_ERR_NOMEM : PDM_ERR_CUDA;  \
+        }                                                                           \
+    } while (0)
+
+extern "C" const char *pdm_strerror(int code)
+{
+    switch (code) {
+    case PDM_OK: return "ok";
+    case PDM_ERR_INVALID_ARG: return "invalid argument";
+    case PDM_ERR_TABLE_RANGE: return "omega*dz/(v*du) exceeds the last table row";
+    case PDM_ERR_TABLE_ASYMMETRIC: return "filter table is not bitwise symmetric in k";
+    case PDM_ERR_UNSUPPORTED: return "unsupported device, path or filter length";
+    case PDM_ERR_NOMEM: return "out of memory";
+    case PDM_ERR_CUDA: return "CUDA call failed (see pdm_info.last_cuda_error)";
+    default: return "unknown pdm_status";
+    }
+}
+
+// R3: q32 = fl32(dz / (v * du)), one rounding from double.
+static inline float host_q(double dz, float v, double du) { return (float)(dz / ((double)v * du)); }
+// R3: FLOAT product (no addend, so no contraction), round half to even, clamp.
+static inline int host_index(float w, float q, int ntab)
+{
+    volatile float prod = w * q;
+    long j = lrintf(prod);
+    if (j < 0) j = 0;
+    if (j > ntab - 1) j = ntab - 1;
+    return (int)j;
+}
+
+static void free_plan(pdm_plan *p)
+{
+    if (!p) return;
+    cudaFree(p->d_omega); cudaFree(p->d_q); cudaFree(p->d_table); cudaFree(p->d_half);
+    cudaFree(p->d_rowoff); cudaFree(p->d_rows); cudaFree(p->d_partial);
+    cudaFree(p->d_plane[0]); cudaFree(p->d_plane[1]); cudaFree(p->d_flags);
+    cudaFree(p->d_stage_p0); cudaFree(p->d_stage_img);
+    delete p;
+}
+
+template <class T>
+static int dev_alloc(pdm_plan *p, T **ptr, size_t count)
+{
+    *ptr = nullptr;
+    if (count == 0) count = 1;
+    PDM_CUDA(p, cudaMalloc((void **)ptr, count * sizeof(T)));
+    p->workspace_bytes += (double)(count * sizeof(T));
+    return PDM_OK;
+}
+
+template <class T>
+static int dev_upload(pdm_plan *p, T **ptr, const T *host, size_t count)
+{
+    int rc = dev_alloc(p, ptr, count);
+    if (rc != PDM_OK) return rc;
+    PDM_CUDA(p, cudaMemcpy(*ptr, host, count * sizeof(T), cudaMemcpyHostToDevice));
+    return PDM_OK;
+}
+
+static int build_plan(pdm_plan *p, const float *omega, const float *velocity, const pdm_c64 *table);
+
+extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, float dz,
+                          const float *omega, const float *velocity,
+                          const pdm_c64 *table, int ntab, int ntaps, double tab_du, unsigned flags)
+{
+    if (!out) return PDM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!omega || !velocity || !table) return PDM_ERR_INVALID_ARG;
+    if (nx <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0)
+        return PDM_ERR_INVALID_ARG;
+    if (!(tab_du > 0.0) || !std::isfinite(tab_du) || !(dz > 0.f) || !std::isfinite(dz) ||
+        !(dx > 0.f) || !std::isfinite(dx))
+        return PDM_ERR_INVALID_ARG;
+    if (flags & ~PDM_FLAGS_VALID) return PDM_ERR_INVALID_ARG;
+    const unsigned path = flags & PDM_PATH_MASK;
+    if (path > PDM_PATH_CLUSTER) return PDM_ERR_INVALID_ARG;
+    if (ntaps > PDM_MAX_TAPS) return PDM_ERR_UNSUPPORTED;
+    if ((double)nz * (double)nx > 2.0e9 || (double)nw * (double)nx > 2.0e9) return PDM_ERR_UNSUPPORTED;
+    for (int i = 0; i < nw; ++i)
+        if (!(omega[i] > 0.f) || !std::isfinite(omega[i])) return PDM_ERR_INVALID_ARG;
+    const size_t plane = (size_t)nz * nx;
+    for (size_t i = 0; i < plane; ++i)
+        if (!(velocity[i] > 0.f) || !std::isfinite(velocity[i])) return PDM_ERR_INVALID_ARG;
+    const int L = (ntaps - 1) / 2;
+    for (int j = 0; j < ntab; ++j) {
+        const pdm_c64 *row = table + (size_t)j * ntaps + L;
+        for (int k = 1; k <= L; ++k)
+            if (memcmp(&row[k], &row[-k], sizeof(pdm_c64)) != 0) return PDM_ERR_TABLE_ASYMMETRIC;
+    }
+
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return PDM_ERR_UNSUPPORTED;           // no usable CUDA device: fail loudly, no fallback
+    }
+    if (prop.major != 10) return PDM_ERR_UNSUPPORTED;
+
+    pdm_plan *p = new (std::nothrow) pdm_plan();
+    if (!p) return PDM_ERR_NOMEM;
+    memset(p, 0, sizeof(*p));
+    p->nx = nx; p->nz = nz; p->nw = nw; p->ntab = ntab; p->ntaps = ntaps; p->L = L;
+    p->dx = dx; p->dz = dz; p->du = tab_du; p->flags = flags;
+    p->device = dev; p->sm_count = prop.multiProcessorCount;
+    p->smem_optin = (int)prop.sharedMemPerBlockOptin;
+
+    int rc = build_plan(p, omega, velocity, table);
+    if (rc != PDM_OK) { free_plan(p); return rc; }
+    *out = p;
+    return PDM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// kernel dispatch: filter half-lengths with a fully unrolled, register-tiled instantiation
+// ------------------------------------------------------------------------------------------------
+#define PDM_R 8
+typedef void (*march_fn)(const pdm_march_params);
+typedef void (*tiled_fn)(const pdm_tiled_params);
+
+#define PDM_FOR_EACH_L(X) X(1) X(2) X(3) X(7) X(12) X(15) X(17) X(25)
+
+static march_fn march_kernel_for(int L, bool taps_smem)
+{
+    switch (L) {
+#define X(LL) case LL: return taps_smem ? pdm_march_kernel<LL, PDM_R, true> : pdm_march_kernel<LL, PDM_R, false>;
+        PDM_FOR_EACH_L(X)
+#undef X
+    default: return nullptr;
+    }
+}
+static tiled_fn tiled_kernel_for(int L)
+{
+    switch (L) {
+#define X(LL) case LL: return pdm_tiled_step<LL, PDM_R>;
+        PDM_FOR_EACH_L(X)
+#undef X
+    default: return nullptr;
+    }
+}
+static int halo_groups(int L, int R) { return (L + 1 + R - 1) / R; }
+static int round_up(int a, int b) { return (a + b - 1) / b * b; }
+
+static int build_plan(pdm_plan *p, const float *omega, const float *velocity, const pdm_c64 *table)
+{
+    const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, ntaps = p->ntaps, L = p->L;
+    const int R = PDM_R;
+    p->R = R;
+
+    // ---- q map (R3) and its extrema ---------------------------------------------------------
+    p->qstride = round_up(nx, PDM_TILED_THREADS * R);
+    std::vector<float> q((size_t)nz * p->qstride);
+    float qmin = INFINITY, qmax = 0.f;
+    for (int z = 0; z < nz; ++z) {
+        float *row = q.data() + (size_t)z * p->qstride;
+        for (int x = 0; x < nx; ++x) {
+            const float v = host_q((double)p->dz, velocity[(size_t)z * nx + x], p->du);
+            row[x] = v;
+            qmin = std::min(qmin, v); qmax = std::max(qmax, v);
+        }
+        for (int x = nx; x < p->qstride; ++x) row[x] = row[nx - 1];
+    }
+    if (!std::isfinite(qmax) || !(qmin > 0.f)) return PDM_ERR_INVALID_ARG;
+    float wmax = 0.f;
+    for (int i = 0; i < nw; ++i) wmax = std::max(wmax, omega[i]);
+    {
+        volatile float prod = wmax * qmax;                 // fl32 product is monotone in both factors
+        if (!(prod < 2.0e9f) || lrintf(prod) > ntab - 1) return PDM_ERR_TABLE_RANGE;
+    }
+
+    // ---- half table: rows k = 0..L as float4 pairs (W_2t, W_2t+1), odd number of float4 per row
+    p->half16 = ((L + 2) / 2) | 1;
+    std::vector<float4> half((size_t)ntab * p->half16, make_float4(0.f, 0.f, 0.f, 0.f));
+    for (int j = 0; j < ntab; ++j)
+        for (int k = 0; k <= L; ++k) {
+            const pdm_c64 w = table[(size_t)j * ntaps + L + k];
+            float4 &d = half[(size_t)j * p->half16 + k / 2];
+            if (k & 1) { d.z = w.re; d.w = w.im; } else { d.x = w.re; d.y = w.im; }
+        }
+
+    // ---- per-omega list of rows that omega can touch ---------------------------------------------
+    // few distinct q (piecewise-constant models): exact compact lists; else the full range [jmin,jmax]
+    std::vector<float> uq;
+    {
+        const size_t cap = 2048;
+        std::vector<float> seen;                           // tiny sorted set with early exit
+        bool few = true;
+        float last = -1.f;
+        for (int z = 0; z < nz && few; ++z) {
+            const float *row = q.data() + (size_t)z * p->qstride;
+            for (int x = 0; x < nx; ++x) {
+                const float v = row[x];
+                if (v == last) continue;
+                last = v;
+                auto it = std::lower_bound(seen.begin(), seen.end(), v);
+                if (it != seen.end() && *it == v) continue;
+                seen.insert(it, v);
+                if (seen.size() > cap) { few = false; break; }
+            }
+        }
+        if (few) uq.swap(seen);
+    }
+    p->contiguous_rows = uq.empty() ? 1 : 0;
+    std::vector<int> rowoff(nw + 1, 0), rows;
+    p->max_rows = 0;
+    for (int i = 0; i < nw; ++i) {
+        size_t before = rows.size();
+        if (p->contiguous_rows) {
+            const int j0 = host_index(omega[i], qmin, ntab), j1 = host_index(omega[i], qmax, ntab);
+            for (int j = j0; j <= j1; ++j) rows.push_back(j);
+        } else {
+            int last = -1;                                 // uq is sorted and the index is monotone in q
+            for (float v : uq) {
+                const int j = host_index(omega[i], v, ntab);
+                if (j != last) { rows.push_back(j); last = j; }
+            }
+        }
+        p->max_rows = std::max(p->max_rows, (int)(rows.size() - before));
+        rowoff[i + 1] = (int)rows.size();
+    }
+
+    // ---- choose the kernel form ----------------------------------------------------------------------
+    const unsigned want = p->flags & PDM_PATH_MASK;
+    const unsigned want_taps = p->flags & PDM_TAPS_MASK;
+    const bool have_L = march_kernel_for(L, false) != nullptr;
+    const int HG = halo_groups(L, R);
+    const int ngroups = (nx + R - 1) / R;
+    const int slots = (2 * HG + ngroups) * (R + 2);
+    const int map_len = round_up(ntab, 8);
+    const size_t line_bytes = (size_t)2 * slots * sizeof(float2) + (size_t)map_len * 2;
+    const size_t slice_bytes = (size_t)p->max_rows * p->half16 * sizeof(float4);
+    const bool lines_fit = have_L && line_bytes <= (size_t)p->smem_optin;
+    const bool slice_fits = lines_fit && line_bytes + slice_bytes <= (size_t)p->smem_optin &&
+                            p->max_rows <= 65535;
+
+    if (want == PDM_PATH_CLUSTER) return PDM_ERR_UNSUPPORTED;       // not built in this round
+    if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
+    if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;
+    if (want == PDM_PATH_AUTO) p->path = lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE);
+    else p->path = (int)want;
+
+    int rc;
+    if ((rc = dev_upload(p, &p->d_omega, omega, (size_t)nw)) != PDM_OK) return rc;
+    if ((rc = dev_upload(p, &p->d_q, q.data(), q.size())) != PDM_OK) return rc;
+
+    if (p->path == PDM_PATH_SMEM) {
+        if (want_taps == PDM_TAPS_SLICE || want_taps == PDM_TAPS_COMPACT) {
+            if (!slice_fits) return PDM_ERR_UNSUPPORTED;
+            p->taps_in_smem = 1;
+        } else if (want_taps == PDM_TAPS_GLOBAL) p->taps_in_smem = 0;
+        else p->taps_in_smem = slice_fits ? 1 : 0;
+        p->taps_mode = p->taps_in_smem ? (p->contiguous_rows ? 2 : 3) : 1;
+
+        int passes = (ngroups + PDM_MARCH_MAX_THREADS - 1) / PDM_MARCH_MAX_THREADS;
+        int threads = round_up((ngroups + passes - 1) / passes, 32);
+        const unsigned tsel = (p->flags >> PDM_THREADS_SHIFT) & 0xFFu;
+        if (tsel) {
+            threads = std::min((int)tsel * 32, PDM_MARCH_MAX_THREADS);
+            passes = (ngroups + threads - 1) / threads;
+        }
+        p->threads = threads;
+        p->smem_bytes = (int)(line_bytes + (p->taps_in_smem ? slice_bytes : 0));
+        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0);
+        PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         p->smem_bytes));
+        int per_sm = 0;
+        PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, threads,
+                                                                  (size_t)p->smem_bytes));
+        if (per_sm < 1) return PDM_ERR_UNSUPPORTED;
+        const unsigned csel = (p->flags >> PDM_CTAS_SHIFT) & 0xFu;
+        if (csel) per_sm = std::min(per_sm, (int)csel);
+        p->ctas_per_sm = per_sm;
+        p->grid = std::min(nw, p->sm_count * per_sm);
+        p->launches = 2;
+        p->n_partial = p->grid;
+        if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->n_partial * nz * (ngroups * R))) != PDM_OK) return rc;
+    } else if (p->path == PDM_PATH_TILED) {
+        p->taps_mode = 1;
+        p->threads = PDM_TILED_THREADS;
+        p->tile_x = PDM_TILED_THREADS * R;
+        const int xtiles = (nx + p->tile_x - 1) / p->tile_x;
+        int wgroups = std::max(1, std::min(nw, (4 * p->sm_count + xtiles - 1) / xtiles));
+        const int wpg = (nw + wgroups - 1) / wgroups;
+        wgroups = (nw + wpg - 1) / wpg;
+        p->wgroups = wgroups;
+        p->grid = xtiles * wgroups;
+        p->ctas_per_sm = 2;
+        p->smem_bytes = (PDM_TILED_THREADS + 2 * HG) * (R + 2) * (int)sizeof(float2);
+        p->launches = nz + 1;
+        p->n_partial = wgroups;
+        tiled_fn fn = tiled_kernel_for(L);
+        PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         p->smem_bytes));
+        if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_partial, (size_t)wgroups * nz * p->qstride)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_plane[0], (size_t)nw * nx)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_plane[1], (size_t)nw * nx)) != PDM_OK) return rc;
+    } else {                                                        // PDM_PATH_NAIVE
+        p->taps_mode = 1;
+        p->threads = 128;
+        p->grid = ((nx + 127) / 128) * nw;
+        p->launches = 2 * nz;
+        if ((rc = dev_upload(p, &p->d_table, reinterpret_cast<const float2 *>(table),
+                             (size_t)ntab * ntaps)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_plane[0], (size_t)nw * nx)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_plane[1], (size_t)nw * nx)) != PDM_OK) return rc;
+    }
+    return PDM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// pdm_migrate: enqueue only -- no allocation, no host sync, no copies (CUDA-graph capturable)
+// ------------------------------------------------------------------------------------------------
+extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev, void *cuda_stream)
+{
+    if (!p || !P0_dev || !image_dev) return PDM_ERR_INVALID_ARG;
+    int dev = -1;
+    PDM_CUDA(p, cudaGetDevice(&dev));
+    if (dev != p->device) { p->last_cuda_error = (int)cudaErrorInvalidDevice; return PDM_ERR_CUDA; }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int nx = p->nx, nz = p->nz, nw = p->nw, L = p->L, R = p->R;
+    const float2 *P0 = reinterpret_cast<const float2 *>(P0_dev);
+
+    if (p->path == PDM_PATH_SMEM) {
+        pdm_march_params a;
+        a.P0 = P0; a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega;
+        a.half = p->d_half; a.rowoff = p->d_rowoff; a.rows = p->d_rows;
+        a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
+        a.ngroups = (nx + R - 1) / R;
+        a.qstride = p->qstride; a.pstride = a.ngroups * R; a.half16 = p->half16;
+        a.passes = (a.ngroups + p->threads - 1) / p->threads;
+        a.slots = (2 * halo_groups(L, R) + a.ngroups) * (R + 2);
+        a.map_len = round_up(p->ntab, 8);
+        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0);
+        fn<<<p->grid, p->threads, p->smem_bytes, st>>>(a);
+        PDM_CUDA(p, cudaGetLastError());
+        dim3 rg((nx + 255) / 256, nz);
+        pdm_reduce_partials<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->n_partial, nz, nx, a.pstride);
+        PDM_CUDA(p, cudaGetLastError());
+    } else if (p->path == PDM_PATH_TILED) {
+        pdm_tiled_params a;
+        a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega; a.half = p->d_half;
+        a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
+        a.qstride = p->qstride; a.pstride = p->qstride; a.half16 = p->half16;
+        a.w_per_group = (nw + p->wgroups - 1) / p->wgroups;
+        tiled_fn fn = tiled_kernel_for(L);
+        dim3 grid((nx + p->tile_x - 1) / p->tile_x, p->wgroups);
+        const float2 *src = P0;
+        for (int z = 0; z < nz; ++z) {
+            a.z = z; a.Pin = src; a.Pout = p->d_plane[z & 1];
+            fn<<<grid, PDM_TILED_THREADS, p->smem_bytes, st>>>(a);
+            src = a.Pout;
+        }
+        PDM_CUDA(p, cudaGetLastError());
+        dim3 rg((nx + 255) / 256, nz);
+        pdm_reduce_partials<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->n_partial, nz, nx, a.pstride);
+        PDM_CUDA(p, cudaGetLastError());
+    } else {
+        dim3 g1((nx + 127) / 128, nw), g2((nx + 127) / 128);
+        const float2 *src = P0;
+        for (int z = 0; z < nz; ++z) {
+            float2 *dst = p->d_plane[z & 1];
+            pdm_naive_step<<<g1, 128, 0, st>>>(src, dst, p->d_omega, p->d_q + (size_t)z * p->qstride,
+                                                p->d_table, nx, nw, p->ntab, L);
+            pdm_naive_image_row<<<g2, 128, 0, st>>>(dst, image_dev + (size_t)z * nx, nx, nw);
+            src = dst;
+        }
+        PDM_CUDA(p, cudaGetLastError());
+    }
+    return PDM_OK;
+}
+
+extern "C" int pdm_migrate_host(pdm_plan *p, const pdm_c64 *P0_host, float *image_host, void *cuda_stream)
+{
+    if (!p || !P0_host || !image_host) return PDM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t nP = (size_t)p->nw * p->nx, nI = (size_t)p->nz * p->nx;
+    if (!p->d_stage_p0) {
+        int rc;
+        if ((rc = dev_alloc(p, &p->d_stage_p0, nP)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_stage_img, nI)) != PDM_OK) return rc;
+    }
+    PDM_CUDA(p, cudaMemcpyAsync(p->d_stage_p0, P0_host, nP * sizeof(pdm_c64), cudaMemcpyHostToDevice, st));
+    int rc = pdm_migrate(p, p->d_stage_p0, p->d_stage_img, cuda_stream);
+    if (rc != PDM_OK) return rc;
+    PDM_CUDA(p, cudaMemcpyAsync(image_host, p->d_stage_img, nI * sizeof(float), cudaMemcpyDeviceToHost, st));
+    PDM_CUDA(p, cudaStreamSynchronize(st));
+    return PDM_OK;
+}
+
+extern "C" int pdm_destroy(pdm_plan *p)
+{
+    free_plan(p);
+    return PDM_OK;
+}
+
+extern "C" int pdm_get_info(const pdm_plan *p, pdm_info *out)
+{
+    if (!p || !out) return PDM_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    out->path = p->path; out->taps_mode = p->taps_mode;
+    out->nx = p->nx; out->nz = p->nz; out->nw = p->nw; out->ntab = p->ntab; out->ntaps = p->ntaps;
+    out->grid_ctas = p->grid; out->threads_per_cta = p->threads; out->ctas_per_sm = p->ctas_per_sm;
+    out->smem_bytes = p->smem_bytes; out->launches_per_migrate = p->launches;
+    out->sm_count = p->sm_count; out->last_cuda_error = p->last_cuda_error;
+    out->samples = (double)p->nx * (double)p->nz * (double)p->nw;
+    out->counted_flops = 8.0 * p->ntaps * out->samples;
+    out->executed_lane_ops = (6.0 * p->L + 4.0) * out->samples;
+    out->workspace_bytes = p->workspace_bytes;
+    return PDM_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// debug / measurement entry points
+// ------------------------------------------------------------------------------------------------
+__global__ void pdm_debug_index_kernel(const float *w, const float *q, int n, int ntab, int *out)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) out[i] = pdm_index(w[i], q[i], ntab - 1);
+}
+
+extern "C" int pdm_debug_table_index(const float *omega, const float *velocity, int n,
+                                     double dz, double tab_du, int ntab, int *idx_out)
+{
+    if (!omega || !velocity || !idx_out || n <= 0 || ntab <= 0 || !(tab_du > 0.0)) return PDM_ERR_INVALID_ARG;
+    std::vector<float> q(n);
+    for (int i = 0; i < n; ++i) q[i] = host_q(dz, velocity[i], tab_du);
+    float *dw = nullptr, *dq = nullptr; int *di = nullptr;
+    int rc = PDM_ERR_CUDA;
+    if (cudaMalloc(&dw, n * sizeof(float)) == cudaSuccess && cudaMalloc(&dq, n * sizeof(float)) == cudaSuccess &&
+        cudaMalloc(&di, n * sizeof(int)) == cudaSuccess &&
+        cudaMemcpy(dw, omega, n * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess &&
+        cudaMemcpy(dq, q.data(), n * sizeof(float), cudaMemcpyHostToDevice) == cudaSuccess) {
+        pdm_debug_index_kernel<<<(n + 255) / 256, 256>>>(dw, dq, n, ntab, di);
+        if (cudaMemcpy(idx_out, di, n * sizeof(int), cudaMemcpyDeviceToHost) == cudaSuccess) rc = PDM_OK;
+    }
+    cudaFree(dw); cudaFree(dq); cudaFree(di);
+    if (rc != PDM_OK) cudaGetLastError();
+    return rc;
+}
+
+extern "C" int pdm_fp32_peak(int packed, int iters, int repeats, void *cuda_stream, double *tflops_out)
+{
+    if (!tflops_out || iters <= 0 || repeats <= 0) return PDM_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return PDM_ERR_UNSUPPORTED;
+    }
+    float *d = nullptr;
+    cudaEvent_t e0, e1;
+    if (cudaMalloc(&d, 256) != cudaSuccess) return PDM_ERR_NOMEM;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int grid = sms * 8, block = 256;
+    double best_ms = 1e30;
+    for (int r = 0; r < repeats + 1; ++r) {                 // first run is the warm-up
+        cudaEventRecord(e0, st);
+        if (packed) pdm_peak_kernel<1><<<grid, block, 0, st>>>(d, iters, 1.0f);
+        else        pdm_peak_kernel<0><<<grid, block, 0, st>>>(d, iters, 1.0f);
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); cudaFree(d); return PDM_ERR_CUDA; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (r > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    const double flops = (double)grid * block * (double)iters * PDM_PEAK_CHAINS * 2.0 * 2.0;
+    *tflops_out = flops / (best_ms * 1e-3) / 1e12;
+    return PDM_OK;
+}

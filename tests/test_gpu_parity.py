@@ -1,0 +1,238 @@
+"""GPU parity: the CUDA path (through the C ABI) against the FP64 oracle, element by element.
+
+Bar (BASELINE.json north_star): relative L2 error <= 1e-4 over the whole image and per-pixel
+error <= 1e-3 of the image maximum.  The table index is taken in FP32 on both sides (reading
+R3), so the only differences are FP32 rounding and summation order (reading R13).
+"""
+import numpy as np
+import pytest
+
+import oracle
+import pdm_inputs
+
+pytestmark = pytest.mark.gpu
+
+REL_L2_BAR = 1e-4
+MAX_PIX_BAR = 1e-3
+
+
+@pytest.fixture(scope="module")
+def pdm():
+    import torch
+    import paper_1912_05529_b200 as m
+    assert torch.cuda.is_available(), "gpu tests need a B200"
+    m.load_library()           # raises if libpdm.so is missing: no fallback
+    return m
+
+
+def errors(gpu_img, ref):
+    g = np.asarray(gpu_img, dtype=np.float64)
+    d = g - ref
+    rel = np.linalg.norm(d) / max(np.linalg.norm(ref), 1e-300)
+    mx = np.abs(d).max() / max(np.abs(ref).max(), 1e-300)
+    return rel, mx
+
+
+def gpu_migrate(pdm, cfg, flags=0, P0=None, want_info=False):
+    import torch
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        p0 = torch.from_numpy(np.ascontiguousarray(cfg["P0"] if P0 is None else P0)).cuda()
+        img = plan.migrate(p0)
+        torch.cuda.synchronize()
+        out = img.cpu().numpy()
+        info = plan.info
+    return (out, info) if want_info else out
+
+
+def assert_parity(pdm, cfg, flags=0, ref=None, expect_path=None):
+    img, info = gpu_migrate(pdm, cfg, flags, want_info=True)
+    if expect_path is not None:
+        assert info["path"] == expect_path, info
+    ref = oracle.migrate(cfg) if ref is None else ref
+    rel, mx = errors(img, ref)
+    assert np.isfinite(img).all()
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (cfg["name"], flags, rel, mx, info)
+    return rel, mx
+
+
+PATHS = ["naive", "smem_global", "smem_staged", "tiled"]
+
+
+def path_flags(pdm, name):
+    return {"naive": pdm.PDM_PATH_NAIVE,
+            "smem_global": pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_GLOBAL,
+            "smem_staged": pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_SLICE,
+            "tiled": pdm.PDM_PATH_TILED}[name]
+
+
+# ---------------------------------------------------------------- every kernel form, small inputs
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps", [
+    ("field", 300, 40, 7, 15),        # ragged tail: nx not a multiple of the 8-sample group
+    ("white", 1000, 24, 5, 25),       # every sample its own table row (general gather path)
+    ("layers", 2500, 30, 6, 31),      # warp-uniform rows; several tiles in the tiled form
+    ("const", 129, 50, 3, 35),        # one sample past a group boundary
+    ("field", 4100, 12, 4, 51),       # two passes per depth step in the SMEM form, 3 x-tiles
+])
+def test_every_path_matches_oracle(pdm, path, model, nx, nz, nw, ntaps):
+    cfg = pdm_inputs.random_problem(11, nx, nz, nw, ntaps, model=model)
+    assert_parity(pdm, cfg, path_flags(pdm, path))
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("L", [1, 2, 3])
+def test_short_filters_and_tiny_grids(pdm, path, L):
+    for seed, nx in ((1, 9), (2, 1), (3, 17), (4, 64)):
+        cfg = pdm_inputs.tiny_random_problem(seed, nx=nx, nz=5, nw=3, L=L, ntab=9)
+        assert_parity(pdm, cfg, path_flags(pdm, path))
+
+
+def test_filter_length_without_unrolled_kernel_uses_scaffold(pdm):
+    cfg = pdm_inputs.tiny_random_problem(7, nx=40, nz=6, nw=3, L=5, ntab=11)   # 11 taps: no instantiation
+    assert_parity(pdm, cfg, 0, expect_path=pdm.PDM_PATH_NAIVE)
+    rc, h = pdm.pdm_create(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"],
+                           cfg["velocity"], cfg["table"], cfg["du"], pdm.PDM_PATH_SMEM)
+    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
+
+
+# ---------------------------------------------------------------- BASELINE.json configs
+def test_config0_all_paths(pdm, config0):
+    ref = oracle.migrate(config0)
+    for path in PATHS:
+        assert_parity(pdm, config0, path_flags(pdm, path), ref=ref)
+    assert_parity(pdm, config0, 0, ref=ref, expect_path=pdm.PDM_PATH_SMEM)
+
+
+def test_config1_auto_and_tiled(pdm):
+    cfg = pdm_inputs.make_config(1)
+    ref = oracle.migrate(cfg)
+    assert_parity(pdm, cfg, 0, ref=ref, expect_path=pdm.PDM_PATH_SMEM)
+    assert_parity(pdm, cfg, pdm.PDM_PATH_TILED, ref=ref)
+
+
+@pytest.mark.slow
+def test_config2_full(pdm):
+    cfg = pdm_inputs.make_config(2)
+    assert_parity(pdm, cfg, 0, expect_path=pdm.PDM_PATH_SMEM)
+
+
+def _subset_parity(pdm, cfg, lines, flags=0, expect_path=None):
+    """Full-size launch configuration, sampled frequencies: P0 is zero except on `lines`, so the
+    image is the sum of exactly those lines' contributions, which the oracle computes one by one."""
+    P0 = np.zeros_like(cfg["P0"])
+    P0[lines] = cfg["P0"][lines]
+    img, info = gpu_migrate(pdm, cfg, flags, P0=P0, want_info=True)
+    if expect_path is not None:
+        assert info["path"] == expect_path
+    ref = oracle.migrate(cfg, omega_index=np.asarray(lines, dtype=np.int32))
+    rel, mx = errors(img, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (cfg["name"], rel, mx, info)
+
+
+@pytest.mark.slow
+def test_config3_full_size_sampled_frequencies(pdm):
+    cfg = pdm_inputs.make_config(3)
+    nw = cfg["nw"]
+    lines = sorted({0, 1, nw // 7, nw // 2, nw - 150, nw - 2, nw - 1})
+    _subset_parity(pdm, cfg, lines, 0, expect_path=pdm.PDM_PATH_SMEM)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("nx,nw,ntaps", [(1024, 64, 15), (4096, 256, 25), (32768, 64, 51), (16384, 64, 15)])
+def test_config4_points_sampled_frequencies(pdm, nx, nw, ntaps):
+    cfg = pdm_inputs.sweep_point(nx, nw, ntaps)
+    lines = sorted({0, nw // 3, nw - 1})
+    _subset_parity(pdm, cfg, lines, 0,
+                   expect_path=pdm.PDM_PATH_TILED if nx >= 16384 else pdm.PDM_PATH_SMEM)
+
+
+# ---------------------------------------------------------------- properties of the GPU path itself
+def test_delta_table_is_identity_on_gpu(pdm):
+    cfg = pdm_inputs.random_problem(3, 520, 9, 4, 25, model="field")
+    cfg = dict(cfg, table=pdm_inputs.filters.delta_table(cfg["ntab"], cfg["ntaps"]))
+    want = cfg["P0"].real.astype(np.float64).sum(axis=0)
+    for path in PATHS:
+        img = gpu_migrate(pdm, cfg, path_flags(pdm, path))
+        for z in range(cfg["nz"]):
+            np.testing.assert_allclose(img[z], want, rtol=0, atol=1e-5)
+
+
+def test_repeated_migrate_is_bit_identical_and_plans_are_independent(pdm):
+    import torch
+    a = pdm_inputs.random_problem(21, 700, 20, 300, 15, model="field")
+    b = pdm_inputs.random_problem(22, 333, 10, 5, 25, model="layers")
+    with pdm.Plan.from_config(a) as pa, pdm.Plan.from_config(b) as pb:
+        xa = torch.from_numpy(a["P0"]).cuda(); xb = torch.from_numpy(b["P0"]).cuda()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            ia1 = pa.migrate(xa, stream=s)
+            ib = pb.migrate(xb, stream=s)
+            ia2 = pa.migrate(xa, stream=s).clone()
+        s.synchronize()
+        ia3 = pa.migrate(xa)
+        torch.cuda.synchronize()
+        assert torch.equal(ia1, ia2) and torch.equal(ia1, ia3)
+        rel, mx = errors(ib.cpu().numpy(), oracle.migrate(b))
+        assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR
+        rel, mx = errors(ia1.cpu().numpy(), oracle.migrate(a))
+        assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR
+
+
+def test_migrate_host_equals_device_call(pdm):
+    import torch
+    cfg = pdm_inputs.random_problem(31, 600, 16, 9, 31, model="field")
+    with pdm.Plan.from_config(cfg) as plan:
+        dev = plan.migrate(torch.from_numpy(cfg["P0"]).cuda())
+        torch.cuda.synchronize()
+        pinned = torch.from_numpy(cfg["P0"]).pin_memory()
+        host = plan.migrate_host(pinned)
+        assert np.array_equal(host, dev.cpu().numpy())
+        host2 = plan.migrate_host(cfg["P0"])
+        assert np.array_equal(host2, host)
+
+
+def test_gpu_index_rule_matches_oracle_bit_for_bit(pdm):
+    rng = np.random.default_rng(12)
+    n = 200000
+    ntab, dz, du = 1024, 10.0, 3.1e-3
+    omega = rng.uniform(10.0, 630.0, n).astype(np.float32)
+    vel = rng.uniform(700.0, 2500.0, n).astype(np.float32)
+    # force exact .5 products: q is a power of two, omega a half-integer multiple of 1/q
+    vel[:64] = np.float32(dz / (0.25 * du))
+    omega[:64] = (np.arange(64, dtype=np.float32) + 0.5) * 4.0
+    got = pdm.pdm_debug_table_index(omega, vel, dz, du, ntab)
+    want = np.array([oracle.table_index(omega[i], vel[i], dz, du, ntab) for i in range(0, n, 37)])
+    assert np.array_equal(got[::37], want)
+    want64 = np.array([oracle.table_index(omega[i], vel[i], dz, du, ntab) for i in range(64)])
+    assert np.array_equal(got[:64], want64)
+
+
+def test_error_codes_on_device(pdm):
+    c = pdm_inputs.tiny_random_problem(5, nx=40, nz=4, nw=3, L=2, ntab=9)
+    args = (c["nx"], c["nz"], c["nw"], c["dx"], c["dz"], c["omega"], c["velocity"], c["table"])
+    rc, h = pdm.pdm_create(*args, c["du"] * 0.5)                     # u exceeds the table
+    assert rc == pdm.PDM_ERR_TABLE_RANGE and h is None
+    rc, h = pdm.pdm_create(*args, c["du"], pdm.PDM_PATH_CLUSTER)
+    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
+    big = pdm_inputs.random_problem(1, 40000, 2, 1, 15, model="const")
+    rc, h = pdm.pdm_create(big["nx"], big["nz"], big["nw"], big["dx"], big["dz"], big["omega"],
+                           big["velocity"], big["table"], big["du"], pdm.PDM_PATH_SMEM)
+    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None              # line cannot fit shared memory
+    rc, h = pdm.pdm_create(*args, c["du"])
+    assert rc == pdm.PDM_OK
+    assert pdm.pdm_migrate(h, 0, 0, 0) == pdm.PDM_ERR_INVALID_ARG
+    assert pdm.pdm_destroy(h) == pdm.PDM_OK
+
+
+def test_create_destroy_does_not_leak(pdm):
+    import torch
+    cfg = pdm_inputs.random_problem(41, 2048, 64, 32, 25, model="field")
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    for _ in range(5):
+        with pdm.Plan.from_config(cfg) as plan:
+            plan.migrate(torch.from_numpy(cfg["P0"]).cuda())
+            torch.cuda.synchronize()
+    torch.cuda.empty_cache()
+    free1, _ = torch.cuda.mem_get_info()
+    assert free0 - free1 < 64 << 20
