@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the f-x poststack depth-migration hot path (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (table look-up, FIR extrapolation, depth marching,
+imaging: SURVEY.md 8(a) A1-A7) over one f-x section: one `pdm_migrate` call.  At N = 1 the
+workload is BASELINE.json configs[3] (the configuration the north_star target is quoted on);
+inputs are seeded and synthetic.  Prints ONE JSON line on rank 0.
+
+N > 1 (torchrun): weak scaling.  The job is the configs[3] model with an N-times denser
+frequency list (the DFT bins of an N-times longer record); rank r owns the bins offset by r/N
+(803 lines each, frequencies are independent units) and the partial images are
+summed with one NCCL all-reduce inside the timed step -- the path's only exchange.
+
+--impl reference: times the FP64 CPU oracle (oracle/, as it stands) on the host cores on a
+bounded sample of the same workload (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "extrapolated samples/sec (z*omega*x points/s)"
+UNIT = "samples/s"
+# FP32 peak the guide's unit counts and clocks give: 148 SMs x 128 FP32
+# lanes x 2 flop/FMA x 1.965 GHz max SM clock.  The FFMA-chain microbenchmark (pdm_fp32_peak)
+# reads 71-73 TFLOP/s on this pool; both are reported.
+FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+
+
+def load_workload(k: int, rank: int, world: int) -> dict:
+    import pdm_inputs
+    if k == 3:
+        from pdm_inputs.configs import config3
+        return config3(bin_offset=rank / world if world > 1 else 0.0)
+    cfg = pdm_inputs.make_config(k)
+    if world > 1:                        # small configs: plain round-robin shard of the lines
+        from paper_1912_05529_b200.shard import shard_workload
+        cfg = shard_workload(cfg, rank, world)
+    return cfg
+
+
+def workload_name(k: int, cfg: dict, world: int) -> str:
+    s = (f"configs[{k}] nx={cfg['nx']} nz={cfg['nz']} nw={cfg['nw']} taps={cfg['ntaps']} "
+         f"ntab={cfg['ntab']}")
+    if world > 1:
+        s += f" per rank x {world} ranks (frequency-sharded, image all-reduce)"
+    return s
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 8:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[4:8]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)),
+                "sm_min_mhz": float(min(sm)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------- oracle legs
+def oracle_sample(cfg: dict, lines_per_thread: int = 4):
+    """Time the FP64 oracle, as it stands, on a bounded sample: `lines_per_thread` x threads
+    evenly spaced frequency lines of the workload, all nz depth steps, all nx samples."""
+    import oracle
+    oracle.build()
+    threads = oracle.num_threads()
+    n = min(cfg["nw"], max(1, lines_per_thread * threads))
+    idx = np.unique(np.linspace(0, cfg["nw"] - 1, n).round().astype(np.int32))
+    t0 = time.perf_counter()
+    oracle.migrate(cfg, omega_index=idx)
+    dt = time.perf_counter() - t0
+    samples = float(idx.size) * cfg["nx"] * cfg["nz"]
+    return samples / dt, dt, int(idx.size), threads
+
+
+def run_reference(args, rank: int, world: int):
+    if rank != 0:
+        return
+    cfg = load_workload(args.config, 0, 1)
+    import oracle
+    # size the per-step sample so warmup+steps stay within a few minutes: ~1 line per thread
+    threads = oracle.num_threads()
+    times, sps = [], []
+    for i in range(args.warmup + args.steps):
+        v, dt, nlines, threads = oracle_sample(cfg, lines_per_thread=1)
+        if i >= args.warmup:
+            times.append(dt); sps.append(v)
+    value = float(np.mean(sps))
+    sample = (f"{nlines} evenly spaced omega lines of {cfg['nw']} per step, all nz={cfg['nz']} depth "
+              f"steps, all nx={cfg['nx']} samples")
+    out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)),
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": {"workload": workload_name(args.config, cfg, 1)},
+           "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
+                            "sample": sample},
+           "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+           "gpu_launches": 0}
+    print(json.dumps(out), flush=True)
+
+
+# ------------------------------------------------------------------------------- our arm
+def run_ours(args, rank: int, local_rank: int, world: int):
+    import torch
+    import torch.distributed as dist
+
+    import paper_1912_05529_b200 as pdm
+    from paper_1912_05529_b200.shard import allreduce_image
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    pdm.load_library()                      # raises if libpdm.so was not built
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = load_workload(args.config, rank, world)
+    plan = pdm.Plan.from_config(cfg, args.flags)
+    info = plan.info
+    samples = info["samples"]
+    stream = torch.cuda.current_stream(dev)
+
+    P0 = torch.from_numpy(cfg["P0"]).to(dev)
+    image = torch.empty((cfg["nz"], cfg["nx"]), dtype=torch.float32, device=dev)
+    P0_pinned = torch.from_numpy(cfg["P0"]).pin_memory()
+    image_pinned = torch.empty((cfg["nz"], cfg["nx"]), dtype=torch.float32).pin_memory()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)     # > 126 MB L2
+
+    def step():
+        plan.migrate(P0, image, stream=stream)
+        if world > 1:
+            allreduce_image(image)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    plan.profile(True)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    # ---- device-resident timing: K steps, CUDA events on the launching stream, L2 flushed between
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    main_ms, reduce_ms = [], []
+    barrier()
+    for a, b in ev:
+        flush.zero_()                                    # L2 flush, outside the timed pair
+        a.record(stream)
+        step()
+        b.record(stream)
+        m, r = plan.profile_read()                       # syncs on this step's last kernel event
+        main_ms.append(m); reduce_ms.append(r)
+    barrier()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = torch.tensor([float(sum(step_ms))], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
+    total_ms = float(total_ms.item())
+    plan.profile(False)
+
+    # ---- end to end through the public HOST-buffer call (pinned host memory, copies inside)
+    h2d = cfg["P0"].nbytes
+    d2h = image_pinned.numel() * 4
+    plan.migrate_host(P0_pinned, image_pinned, stream=stream)
+    barrier()
+    e2e_ev = []
+    for _ in range(args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        plan.migrate_host(P0_pinned, image_pinned, stream=stream)   # returns after the D2H copy
+        if world > 1:
+            # the reduced image is what the job returns: reduce on device, then read it back
+            image.copy_(image_pinned, non_blocking=True)
+            allreduce_image(image)
+            image_pinned.copy_(image, non_blocking=True)
+        b.record(stream)
+        e2e_ev.append((a, b))
+    barrier()
+    e2e_ms = torch.tensor([float(sum(a.elapsed_time(b) for a, b in e2e_ev))],
+                          dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(e2e_ms, op=dist.ReduceOp.MAX)
+    e2e_ms = float(e2e_ms.item())
+    clocks = sampler.stop()
+
+    if rank == 0:
+        k = args.steps
+        value = samples * world * k / (total_ms * 1e-3)
+        main_avg = float(np.mean(main_ms))
+        launches_main = info["launches_per_migrate"] - 1 if info["path"] != pdm.PDM_PATH_NAIVE else info["launches_per_migrate"]
+        per_launch_ms = main_avg / max(1, launches_main)
+        flops_per_launch = info["counted_flops"] / max(1, launches_main)
+        achieved = flops_per_launch / (per_launch_ms * 1e-3) / 1e12
+        try:
+            fma_peak = pdm.pdm_fp32_peak(True, 50000, 3, stream.cuda_stream)
+        except pdm.PdmError:
+            fma_peak = None
+        kernel = {pdm.PDM_PATH_SMEM: "pdm_march_kernel", pdm.PDM_PATH_TILED: "pdm_tiled_step",
+                  pdm.PDM_PATH_NAIVE: "pdm_naive_step"}.get(info["path"], "?")
+        roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
+                    "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                    "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
+                    "traffic": None,
+                    "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); "
+                                   "MEASURED_PEAKS.json has no FP32 entry",
+                    "ffma_chain_measured_tflops": fma_peak,
+                    "frac_of_ffma_chain": (achieved / fma_peak) if fma_peak else None,
+                    "flops_counted": "8*(2L+1) per sample (metric definition); the kernel folds "
+                                     "W_k == W_-k and executes (6L+4)/(4(2L+1)) of the lane-ops",
+                    "kernel_ms_per_launch": per_launch_ms, "launches_per_step": launches_main,
+                    "kernel_share_of_step": main_avg / (float(np.mean(step_ms))),
+                    "reduce_ms": float(np.mean(reduce_ms))}
+        cpu_v, cpu_dt, cpu_lines, cpu_threads = oracle_sample(cfg, lines_per_thread=args.cpu_lines_per_thread)
+        out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": k,
+               "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
+               "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+               "config": {"workload": workload_name(args.config, cfg, world),
+                          "path": {1: "smem-marching", 2: "x-tiled", 3: "naive"}.get(info["path"]),
+                          "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
+                          "smem_bytes": info["smem_bytes"],
+                          "l2": "256 MiB buffer written between timed steps (L2 flush); per-step "
+                                f"working set {info['workspace_bytes'] / 1e9:.2f} GB > 126 MB L2"},
+               "pct_fp32_peak_counted": 100.0 * value / world * 8 * cfg["ntaps"] / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+               "roofline": roofline,
+               "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
+                                "sample": f"{cpu_lines} evenly spaced omega lines of {cfg['nw']}, all "
+                                          f"nz={cfg['nz']} steps, all nx={cfg['nx']} samples, "
+                                          f"{cpu_dt:.1f} s wall"},
+               "e2e": {"value": samples * world * k / (e2e_ms * 1e-3), "unit": UNIT,
+                       "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                       "ms_per_step": e2e_ms / k},
+               "gpu_launches": int(info["launches_per_migrate"]) * k,
+               "clocks": clocks}
+        print(json.dumps(out), flush=True)
+    plan.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
+    ap.add_argument("--flags", type=lambda s: int(s, 0), default=0, help="pdm_create flags word")
+    ap.add_argument("--cpu-lines-per-thread", type=int, default=4)
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, local_rank, world)
+
+
+if __name__ == "__main__":
+    main()

@@ -134,6 +134,19 @@ int pdm_get_info(const pdm_plan *plan, pdm_info *out);
 const char *pdm_strerror(int code);
 
 /*
+ * pdm_profile_enable / pdm_profile_read -- per-kernel device timing for the roofline report.
+ * While enabled, pdm_migrate records CUDA events on the caller's stream before the dominant
+ * kernel(s) (A1-A4: the marching kernel, or all nz x-tiled step launches), between them and the
+ * imaging reduction (A5), and after it.  Recording an event is capture-safe and costs ~1 us.
+ * pdm_profile_read synchronises on the last event of the most recent pdm_migrate and returns
+ *   main_ms    HOST float: duration of the dominant kernel(s) of that call, milliseconds
+ *   reduce_ms  HOST float: duration of the reduction kernel
+ * Errors: PDM_ERR_INVALID_ARG (NULL, profiling not enabled or no migrate since), PDM_ERR_CUDA.
+ */
+int pdm_profile_enable(pdm_plan *plan, int enable);
+int pdm_profile_read(pdm_plan *plan, float *main_ms, float *reduce_ms);
+
+/*
  * pdm_debug_table_index -- DEVICE evaluation of the index rule R3 (pin P12 on the GPU side):
  *   idx_dev[i] = clamp(rint(fl32(omega_dev[i] * q)), 0, ntab-1), q = (float)(dz/(velocity_dev[i]*tab_du))
  * with q formed on the HOST side of the library exactly as pdm_create does (so velocity is HOST).

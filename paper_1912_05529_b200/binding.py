@@ -27,7 +27,8 @@ PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 
 PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TILE_SHIFT = 8, 16, 20
 
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
-                    "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak")
+                    "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
+                    "pdm_profile_enable", "pdm_profile_read")
 
 
 class PdmInfo(ctypes.Structure):
@@ -78,6 +79,10 @@ def load_library(path: str | None = None):
     lib.pdm_debug_table_index.argtypes = [vp, vp, ci, cd, cd, ci, vp]
     lib.pdm_fp32_peak.restype = ci
     lib.pdm_fp32_peak.argtypes = [ci, ci, ci, vp, ctypes.POINTER(cd)]
+    lib.pdm_profile_enable.restype = ci
+    lib.pdm_profile_enable.argtypes = [vp, ci]
+    lib.pdm_profile_read.restype = ci
+    lib.pdm_profile_read.argtypes = [vp, ctypes.POINTER(cf), ctypes.POINTER(cf)]
     _lib = lib
     return lib
 
@@ -130,6 +135,19 @@ def pdm_get_info(plan) -> PdmInfo:
     if rc != PDM_OK:
         raise PdmError(rc, "pdm_get_info")
     return info
+
+
+def pdm_profile_enable(plan, enable: bool = True) -> int:
+    return load_library().pdm_profile_enable(plan, int(bool(enable)))
+
+
+def pdm_profile_read(plan):
+    """-> (main_ms, reduce_ms) of the most recent pdm_migrate (synchronises on its last event)."""
+    a, b = ctypes.c_float(), ctypes.c_float()
+    rc = load_library().pdm_profile_read(plan, ctypes.byref(a), ctypes.byref(b))
+    if rc != PDM_OK:
+        raise PdmError(rc, "pdm_profile_read")
+    return float(a.value), float(b.value)
 
 
 def pdm_debug_table_index(omega, velocity, dz, tab_du, ntab) -> np.ndarray:
@@ -215,6 +233,14 @@ class Plan:
         if rc != PDM_OK:
             raise PdmError(rc, "pdm_migrate_host")
         return image_host
+
+    def profile(self, enable: bool = True):
+        rc = pdm_profile_enable(self._h, enable)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_profile_enable")
+
+    def profile_read(self):
+        return pdm_profile_read(self._h)
 
     def close(self):
         if self._h is not None:

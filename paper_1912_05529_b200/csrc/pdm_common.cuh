@@ -38,6 +38,10 @@ struct pdm_plan {
     pdm_c64 *d_stage_p0;
     float   *d_stage_img;
 
+    // ---- pdm_profile_enable: events around the dominant kernel(s) and the reduction -----------------
+    int profiling, profiled;
+    cudaEvent_t ev[3];
+
     // ---- launch configuration ------------------------------------------------------------------
     int R;                // outputs per thread of the register-tiled kernels
     int threads, grid, ctas_per_sm, smem_bytes, launches;

@@ -283,15 +283,21 @@ def faulted_velocity(rng, nz, nx, dz, dx):
     return v
 
 
-def config3(seed: int = BASE_SEED + 3):
-    """Strong contrast: 6144x1500, faulted layers + 4500 m/s body, 2000 diffractors + 5% noise, 51 taps."""
+def config3(seed: int = BASE_SEED + 3, bin_offset: float = 0.0):
+    """Strong contrast: 6144x1500, faulted layers + 4500 m/s body, 2000 diffractors + 5% noise, 51 taps.
+
+    `bin_offset` in [0,1) shifts every frequency by that fraction of a DFT bin: the union over
+    r = 0..N-1 of bin_offset = r/N is the bin set of an N-times longer record, which is how
+    bench.py builds the N-GPU weak-scaling job (one offset per rank; same velocity model).
+    """
     def build():
         rng = np.random.default_rng(seed)
         nx, nz, dx, dz = 6144, 1500, 5.0, 5.0
         nt, dt = 4096, 2e-3
         omega = dft_bin_omegas(nt, dt, 2.0, 100.0)
         domega = 2.0 * np.pi / (nt * dt)
-        j0 = int(np.rint(float(omega[0]) / domega))
+        j0 = int(np.rint(float(omega[0]) / domega)) + float(bin_offset)
+        omega = ((j0 + np.arange(omega.size)) * domega).astype(np.float32)
         v = faulted_velocity(rng, nz, nx, dz, dx)
         x = np.arange(nx) * dx
         nd = 2000
@@ -306,7 +312,8 @@ def config3(seed: int = BASE_SEED + 3):
         noise = rng.standard_normal(P0.shape) + 1j * rng.standard_normal(P0.shape)
         P0 = P0 + (0.05 * rms / np.sqrt(2.0)) * noise
         return dict(omega=omega, v=v.astype(np.float32), P0=P0.astype(np.complex64))
-    d = _cached_npz(f"config3_{seed}", build)
+    tag = f"config3_{seed}" if bin_offset == 0.0 else f"config3_{seed}_off{bin_offset:.6f}"
+    d = _cached_npz(tag, build)
     return _finish("configs[3] 6144x1500 faulted+body", 6144, 1500, 5.0, 5.0, 51,
                    d["omega"], d["v"], d["P0"])
 
