@@ -310,7 +310,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--flags", type=lambda s: int(s, 0), default=0, help="pdm_create flags word")
-    ap.add_argument("--cpu-lines-per-thread", type=int, default=4)
+    ap.add_argument("--cpu-lines-per-thread", type=int, default=16)
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
