@@ -33,6 +33,10 @@ struct pdm_march_params {
     const float4 *half;      // [ntab][half16]
     const int    *rowoff;    // [nw+1]
     const int    *rows;      // row lists
+    const int4   *segs;      // work list: {line, z0, z1, hand-off slot or -1}, in execution order per CTA
+    const int    *segoff;    // [grid+1] offsets into segs
+    float2       *handoff;   // [nslots][nx] wavefield of a line split between two CTAs, at the split depth
+    int          *flags;     // [nslots] 0 = empty, 1 = hand-off line published (reset by the consumer)
     int nx, nz, nw, ntab;
     int qstride, pstride, half16;
     int ngroups, passes, slots, map_len;
@@ -116,10 +120,19 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
         reinterpret_cast<float4 *>(buf_a)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
 
     float *const my_partial = p.partial + (size_t)blockIdx.x * p.nz * p.pstride;
-    bool first = true;
+    // Rows z < wz of my_partial already hold sums of earlier segments; rows >= wz are unwritten.
+    int wz = 0;
 
-    for (int line = blockIdx.x; line < p.nw; line += gridDim.x) {
-        __syncthreads();                                 // previous line (and the zero fill) done
+    // Work list (pdm_create): whole lines, plus -- when depth-split balancing is on -- the HEAD
+    // [0,z1) of one line (done first, then published through `handoff`) and the TAIL [z0,nz) of
+    // another (done last, after the CTA that owns its head has published it).  Every CTA then
+    // marches the same number of depth steps; lines are sequential in z but nothing
+    // says a line must stay on one SM.
+    const int seg_end = p.segoff[blockIdx.x + 1];
+    for (int sidx = p.segoff[blockIdx.x]; sidx < seg_end; ++sidx) {
+        const int4 sg = p.segs[sidx];
+        const int line = sg.x, z0 = sg.y, z1 = sg.z, slot = sg.w;
+        __syncthreads();                                 // previous segment (and the zero fill) done
         const float w = p.omega[line];
         if (TAPS_SMEM) {                                 // A2 staging: rows this omega can touch
             const int r0 = p.rowoff[line], nrows = p.rowoff[line + 1] - r0;
@@ -130,11 +143,28 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                 slice[e] = p.half[(size_t)p.rows[r0 + s] * p.half16 + c];
             }
         }
-        {                                                // P(z=0) = P0[line]
-            const float2 *src = p.P0 + (size_t)line * p.nx;
+        if (z0 > 0) {                                    // TAIL: wait for the head's owner
+            if (wz < p.nz) {                             // no whole line came before: define the rest
+                const int n4 = (p.nz - wz) * (p.pstride / 4);
+                float4 *dstz = reinterpret_cast<float4 *>(my_partial + (size_t)wz * p.pstride);
+                for (int i = tid; i < n4; i += T) dstz[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                wz = p.nz;
+            }
+            if (tid == 0) {
+                unsigned v;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p.flags + slot) : "memory");
+                    if (!v) __nanosleep(200);
+                } while (!v);
+                p.flags[slot] = 0;                       // one producer, one consumer per migrate
+            }
+            __syncthreads();
+        }
+        {                                                // P(z0): P0[line] or the hand-off
+            const float2 *src = (z0 == 0) ? p.P0 + (size_t)line * p.nx : p.handoff + (size_t)slot * p.nx;
             for (int x = tid; x < p.nx; x += T) {
                 const int g = x / R;
-                buf_a[(HG + g) * GS + (x - g * R)] = src[x];
+                buf_a[(HG + g) * GS + (x - g * R)] = __ldcg(src + x);
             }
         }
         __syncthreads();
@@ -143,14 +173,15 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
         float qn[R];
         {
             const int g0 = min(tid, p.ngroups - 1);
-            const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)g0 * R);
+            const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)z0 * p.qstride + (size_t)g0 * R);
 #pragma unroll
             for (int i = 0; i < R / 4; ++i) {
                 const float4 v = __ldg(qp + i);
                 qn[4 * i] = v.x; qn[4 * i + 1] = v.y; qn[4 * i + 2] = v.z; qn[4 * i + 3] = v.w;
             }
         }
-        for (int z = 0; z < p.nz; ++z) {
+        for (int z = z0; z < z1; ++z) {
+            const bool accumulate = z < wz;
             for (int pass = 0; pass < p.passes; ++pass) {
                 const int g_raw = pass * T + tid;
                 // whole warp beyond the line: nothing to do in this pass (warp-uniform)
@@ -161,7 +192,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                 {                                        // A1 prefetch: q of the next (z, pass)
                     int pz = z, pp = pass + 1;
                     if (pp == p.passes) { pp = 0; ++pz; }
-                    if (pz < p.nz) {
+                    if (pz < z1) {
                         const int gn = min(pp * T + tid, p.ngroups - 1);
                         const float4 *qp = reinterpret_cast<const float4 *>(
                             p.q + (size_t)pz * p.qstride + (size_t)gn * R);
@@ -178,7 +209,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
 
                 float4 *prow = reinterpret_cast<float4 *>(my_partial + (size_t)z * p.pstride + (size_t)g * R);
                 float4 pold[R / 4];
-                if (!first) {                            // A5: old partial row, consumed at the end
+                if (accumulate) {                        // A5: old partial row, consumed at the end
 #pragma unroll
                     for (int i = 0; i < R / 4; ++i) pold[i] = __ldcs(prow + i);
                 } else {
@@ -229,7 +260,20 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
             __syncthreads();                             // A4: step z complete for the whole line
             float2 *t = cur; cur = nxt; nxt = t;
         }
-        first = false;
+        if (z0 == 0) wz = max(wz, z1);                   // a head or a whole line defines rows [0,z1)
+        if (z1 < p.nz) {                                 // HEAD: publish the line at depth z1
+            float2 *dst = p.handoff + (size_t)slot * p.nx;
+            for (int x = tid; x < p.nx; x += T) {
+                const int g = x / R;
+                __stcg(dst + x, cur[(HG + g) * GS + (x - g * R)]);
+            }
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) {
+                const unsigned one = 1u;
+                asm volatile("st.release.gpu.global.u32 [%0], %1;" :: "l"(p.flags + slot), "r"(one) : "memory");
+            }
+        }
     }
 }
 

@@ -57,6 +57,7 @@ static void free_plan(pdm_plan *p)
     cudaFree(p->d_omega); cudaFree(p->d_q); cudaFree(p->d_table); cudaFree(p->d_half);
     cudaFree(p->d_rowoff); cudaFree(p->d_rows); cudaFree(p->d_partial);
     cudaFree(p->d_plane[0]); cudaFree(p->d_plane[1]); cudaFree(p->d_flags);
+    cudaFree(p->d_handoff); cudaFree(p->d_segs); cudaFree(p->d_segoff);
     cudaFree(p->d_stage_p0); cudaFree(p->d_stage_img);
     for (int i = 0; i < 3; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
     delete p;
@@ -161,6 +162,45 @@ static tiled_fn tiled_kernel_for(int L)
     default: return nullptr;
     }
 }
+// Work list of the marching kernel.  Unbalanced: CTA c owns whole lines c, c+grid, ...  Balanced
+// (nw >= grid): the nw*nz depth steps, laid end to end line after line, are cut into `grid` equal
+// ranges; a range is [tail of a line][whole lines][head of a line].  The CTA runs its head FIRST
+// (it depends on nothing) and publishes the line at the split depth, its tail LAST (by then the
+// owner of that line's head has long published it), so no CTA waits on work that has not started.
+static void build_segments(int nw, int nz, int grid, bool balance,
+                           std::vector<int4> &segs, std::vector<int> &segoff, int &nslots)
+{
+    segs.clear(); segoff.assign(grid + 1, 0); nslots = 0;
+    if (!balance) {
+        for (int c = 0; c < grid; ++c) {
+            for (int line = c; line < nw; line += grid) segs.push_back(make_int4(line, 0, nz, -1));
+            segoff[c + 1] = (int)segs.size();
+        }
+        return;
+    }
+    const long long total = (long long)nw * nz;
+    std::vector<int> slot_of_line(nw, -1);
+    for (int c = 0; c < grid; ++c) {
+        const long long a = total * c / grid, b = total * (c + 1) / grid;
+        std::vector<int4> mine;
+        for (long long t = a; t < b;) {
+            const int line = (int)(t / nz), z0 = (int)(t - (long long)line * nz);
+            const int z1 = (int)std::min<long long>(nz, z0 + (b - t));
+            if ((z0 > 0 || z1 < nz) && slot_of_line[line] < 0) slot_of_line[line] = nslots++;
+            mine.push_back(make_int4(line, z0, z1, (z0 > 0 || z1 < nz) ? slot_of_line[line] : -1));
+            t += z1 - z0;
+        }
+        // execution order: head (z0 == 0, z1 < nz) first, tail (z0 > 0) last
+        if (!mine.empty() && mine.back().y == 0 && mine.back().z < nz) segs.push_back(mine.back());
+        for (size_t i = 0; i < mine.size(); ++i) {
+            const int4 m = mine[i];
+            if (m.y == 0 && m.z == nz) segs.push_back(m);
+        }
+        if (!mine.empty() && mine.front().y > 0) segs.push_back(mine.front());
+        segoff[c + 1] = (int)segs.size();
+    }
+}
+
 static int halo_groups(int L, int R) { return (L + 1 + R - 1) / R; }
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
@@ -296,6 +336,20 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->grid = std::min(nw, p->sm_count * per_sm);
         p->launches = 2;
         p->n_partial = p->grid;
+        {
+            int coop = 0;
+            PDM_CUDA(p, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device));
+            // a line split needs T = nw*nz/grid >= nz (pieces are heads and tails only) and all
+            // CTAs co-resident (cooperative launch); whole lines per CTA otherwise
+            p->balanced = (!(p->flags & PDM_NO_BALANCE) && coop && nw > p->grid && nw % p->grid != 0) ? 1 : 0;
+            std::vector<int4> segs; std::vector<int> segoff;
+            build_segments(nw, nz, p->grid, p->balanced != 0, segs, segoff, p->nslots);
+            if ((rc = dev_upload(p, &p->d_segs, segs.data(), segs.size())) != PDM_OK) return rc;
+            if ((rc = dev_upload(p, &p->d_segoff, segoff.data(), segoff.size())) != PDM_OK) return rc;
+            if ((rc = dev_alloc(p, &p->d_handoff, (size_t)std::max(1, p->nslots) * nx)) != PDM_OK) return rc;
+            if ((rc = dev_alloc(p, &p->d_flags, (size_t)std::max(1, p->nslots))) != PDM_OK) return rc;
+            PDM_CUDA(p, cudaMemset(p->d_flags, 0, (size_t)std::max(1, p->nslots) * sizeof(int)));
+        }
         if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
@@ -351,6 +405,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         pdm_march_params a;
         a.P0 = P0; a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega;
         a.half = p->d_half; a.rowoff = p->d_rowoff; a.rows = p->d_rows;
+        a.segs = p->d_segs; a.segoff = p->d_segoff; a.handoff = p->d_handoff; a.flags = p->d_flags;
         a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
         a.ngroups = (nx + R - 1) / R;
         a.qstride = p->qstride; a.pstride = a.ngroups * R; a.half16 = p->half16;
@@ -359,7 +414,13 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.map_len = round_up(p->ntab, 8);
         march_fn fn = march_kernel_for(L, p->taps_in_smem != 0);
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
-        fn<<<p->grid, p->threads, p->smem_bytes, st>>>(a);
+        if (p->balanced) {                               // split lines: CTAs wait on one another
+            void *args[] = { (void *)&a };
+            PDM_CUDA(p, cudaLaunchCooperativeKernel((const void *)fn, dim3(p->grid), dim3(p->threads),
+                                                    args, (size_t)p->smem_bytes, st));
+        } else {
+            fn<<<p->grid, p->threads, p->smem_bytes, st>>>(a);
+        }
         PDM_CUDA(p, cudaGetLastError());
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[1], st));
         dim3 rg((nx + 255) / 256, nz);

@@ -32,7 +32,11 @@ struct pdm_plan {
     float  *d_partial;    // march: [n_partial][nz][nx] per-CTA partial images; tiled: [wgroups][nz][nx]
     int     n_partial;
     float2 *d_plane[2];   // tiled/naive: HBM ping-pong planes [nw][nx]
-    int    *d_flags;      // march: depth-split hand-off flags
+    int    *d_flags;      // march: depth-split hand-off flags [nslots]
+    float2 *d_handoff;    // march: [nslots][nx] wavefield of a split line at its split depth
+    int4   *d_segs;       // march: work list {line, z0, z1, slot}, execution order per CTA
+    int    *d_segoff;     // march: [grid+1]
+    int     nslots, balanced;
 
     // ---- pdm_migrate_host staging --------------------------------------------------------------
     pdm_c64 *d_stage_p0;

@@ -95,6 +95,33 @@ def test_filter_length_without_unrolled_kernel_uses_scaffold(pdm):
     assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
 
 
+@pytest.mark.parametrize("nx,nz,nw,ntaps,model,ctas", [
+    (200, 37, 700, 15, "field", 1),     # 148 CTAs, 4.7 lines each: tail + whole lines + head per CTA
+    (520, 23, 151, 25, "layers", 1),    # 1.02 lines each: most CTAs own only a tail and a head
+    (300, 16, 449, 7, "white", 3),      # 444 CTAs (3 per SM), 5 lines over
+])
+def test_depth_split_balancing_matches_oracle_and_whole_line_schedule(pdm, nx, nz, nw, ntaps, model, ctas):
+    """Lines split between CTAs at a depth (hand-off through HBM) give the same image as whole
+    lines per CTA, up to the summation order of the partial images, and both match the oracle."""
+    cfg = pdm_inputs.random_problem(17, nx, nz, nw, ntaps, model=model)
+    ref = oracle.migrate(cfg)
+    base = pdm.PDM_PATH_SMEM | (ctas << pdm.PDM_CTAS_SHIFT)
+    img_b, info_b = gpu_migrate(pdm, cfg, base, want_info=True)
+    img_w, info_w = gpu_migrate(pdm, cfg, base | pdm.PDM_NO_BALANCE, want_info=True)
+    assert info_b["grid_ctas"] == info_w["grid_ctas"] == 148 * ctas
+    for img in (img_b, img_w):
+        rel, mx = errors(img, ref)
+        assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+    # run the balanced plan twice more: the hand-off flags must be back to empty after each call
+    import torch
+    with pdm.Plan.from_config(cfg, base) as plan:
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(p0).clone()
+        torch.cuda.synchronize()
+        assert torch.equal(a, b) and np.array_equal(a.cpu().numpy(), img_b)
+
+
 # ---------------------------------------------------------------- BASELINE.json configs
 def test_config0_all_paths(pdm, config0):
     ref = oracle.migrate(config0)
