@@ -24,6 +24,9 @@
 #include "pdm_common.cuh"
 
 #define PDM_MARCH_MAX_THREADS 384
+#ifndef PDM_FIR_FORM
+#define PDM_FIR_FORM 1
+#endif
 
 struct pdm_march_params {
     const float2 *P0;        // [nw][nx]
@@ -72,8 +75,13 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
 #pragma unroll
     for (int r = 0; r < R; ++r) {                       // centre tap W_0
         const float4 t = tw[UNIFORM ? 0 : r];
+#if PDM_FIR_FORM == 0
         acc_a[r] = pk_mul_s(t.x, wl[r]);
         acc_b[r] = pk_mul_s(t.y, wl[r]);
+#else
+        acc_a[r] = pk_mul_s(wl[r].x, f4lo(t));
+        acc_b[r] = pk_mul_s(wl[r].y, f4lo(t));
+#endif
     }
     float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
 #pragma unroll
@@ -89,6 +97,7 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
 #pragma unroll
             for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r] + k / 2];
         }
+#if PDM_FIR_FORM == 0
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 t = tw[UNIFORM ? 0 : r];
@@ -97,6 +106,40 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
             acc_a[r] = pk_fma_s(wre, s, acc_a[r]);
             acc_b[r] = pk_fma_s(wim, s, acc_b[r]);
         }
+#elif PDM_FIR_FORM == 1
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            const float2 W = (k & 1) ? f4hi(t) : f4lo(t);
+            const float2 s = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
+            acc_a[r] = pk_fma_s(s.x, W, acc_a[r]);
+            acc_b[r] = pk_fma_s(s.y, W, acc_b[r]);
+        }
+#else
+        float2 s[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) s[r] = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
+#if PDM_FIR_FORM == 2
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            acc_a[r] = pk_fma_s(s[r].x, (k & 1) ? f4hi(t) : f4lo(t), acc_a[r]);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            acc_b[r] = pk_fma_s(s[r].y, (k & 1) ? f4hi(t) : f4lo(t), acc_b[r]);
+        }
+#else
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            const float2 W = (k & 1) ? f4hi(t) : f4lo(t);
+            acc_a[r] = pk_fma_s(s[r].x, W, acc_a[r]);
+            acc_b[r] = pk_fma_s(s[r].y, W, acc_b[r]);
+        }
+#endif
+#endif
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
@@ -114,7 +157,14 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
     unsigned short *map = reinterpret_cast<unsigned short *>(buf_b + p.slots);
     float4 *slice = reinterpret_cast<float4 *>(map + p.map_len);
 
+    // A4 without a CTA barrier: prog[1 + w] = depth steps of the current segment that warp w has
+    // completed.  A warp owns `passes` x 32 CONTIGUOUS groups, so step s+1 of warp w reads only
+    // what warps w-1, w, w+1 wrote in step s (halo <= HG groups < 32): it may start as soon as
+    // both neighbours have completed step s, which also covers the write-after-read on the
+    // ping-pong buffer.  prog[0] and prog[nwarps + 1] are sentinels (always ahead).
+    __shared__ int prog[PDM_MARCH_MAX_THREADS / 32 + 2];
     const int tid = threadIdx.x, T = blockDim.x;
+    const int warp = tid >> 5, lane = tid & 31, nwarps = T >> 5;
     const int ntab_m1 = p.ntab - 1;
     for (int i = tid; i < p.slots; i += T)              // 2*slots float2 = slots float4
         reinterpret_cast<float4 *>(buf_a)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -160,6 +210,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
             }
             __syncthreads();
         }
+        if (tid < nwarps + 2) prog[tid] = (tid == 0 || tid == nwarps + 1) ? 0x7fffffff : 0;
         {                                                // P(z0): P0[line] or the hand-off
             const float2 *src = (z0 == 0) ? p.P0 + (size_t)line * p.nx : p.handoff + (size_t)slot * p.nx;
             for (int x = tid; x < p.nx; x += T) {
@@ -172,7 +223,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
         float2 *cur = buf_a, *nxt = buf_b;
         float qn[R];
         {
-            const int g0 = min(tid, p.ngroups - 1);
+            const int g0 = min(warp * p.passes * 32 + lane, p.ngroups - 1);
             const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)z0 * p.qstride + (size_t)g0 * R);
 #pragma unroll
             for (int i = 0; i < R / 4; ++i) {
@@ -183,9 +234,9 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
         for (int z = z0; z < z1; ++z) {
             const bool accumulate = z < wz;
             for (int pass = 0; pass < p.passes; ++pass) {
-                const int g_raw = pass * T + tid;
+                const int g_raw = (warp * p.passes + pass) * 32 + lane;
                 // whole warp beyond the line: nothing to do in this pass (warp-uniform)
-                const bool warp_active = (pass * T + (tid & ~31)) < p.ngroups;
+                const bool warp_active = (warp * p.passes + pass) * 32 < p.ngroups;
                 float qc[R];
 #pragma unroll
                 for (int r = 0; r < R; ++r) qc[r] = qn[r];
@@ -193,7 +244,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                     int pz = z, pp = pass + 1;
                     if (pp == p.passes) { pp = 0; ++pz; }
                     if (pz < z1) {
-                        const int gn = min(pp * T + tid, p.ngroups - 1);
+                        const int gn = min((warp * p.passes + pp) * 32 + lane, p.ngroups - 1);
                         const float4 *qp = reinterpret_cast<const float4 *>(
                             p.q + (size_t)pz * p.qstride + (size_t)gn * R);
 #pragma unroll
@@ -223,6 +274,15 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                 for (int r = 0; r < R; ++r) {
                     j[r] = pdm_index(w, qc[r], ntab_m1);
                     uni = uni && (j[r] == j[0]);
+                }
+                if (pass == 0 && z > z0) {               // A4: neighbours have completed step z-1
+                    if (lane == 0) {
+                        const int need = z - z0;
+                        while (*(volatile int *)&prog[warp] < need) { }
+                        while (*(volatile int *)&prog[warp + 2] < need) { }
+                        __threadfence_block();
+                    }
+                    __syncwarp();
                 }
                 int toff[R];
                 const float4 *tbase = TAPS_SMEM ? slice : p.half;
@@ -257,11 +317,16 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                     }
                 }
             }
-            __syncthreads();                             // A4: step z complete for the whole line
+            __syncwarp();                                // A4: publish this warp's step z
+            if (lane == 0) {
+                __threadfence_block();
+                *(volatile int *)&prog[warp + 1] = z - z0 + 1;
+            }
             float2 *t = cur; cur = nxt; nxt = t;
         }
         if (z0 == 0) wz = max(wz, z1);                   // a head or a whole line defines rows [0,z1)
         if (z1 < p.nz) {                                 // HEAD: publish the line at depth z1
+            __syncthreads();                             // every warp has completed step z1-1
             float2 *dst = p.handoff + (size_t)slot * p.nx;
             for (int x = tid; x < p.nx; x += T) {
                 const int g = x / R;
