@@ -24,9 +24,6 @@
 #include "pdm_common.cuh"
 
 #define PDM_MARCH_MAX_THREADS 384
-#ifndef PDM_FIR_FORM
-#define PDM_FIR_FORM 1
-#endif
 
 struct pdm_march_params {
     const float2 *P0;        // [nw][nx]
@@ -57,6 +54,10 @@ __device__ __forceinline__ float2 f4hi(float4 v) { return make_float2(v.z, v.w);
 // One group of R outputs.  `base` = &line[slot(x0)];  tbase + toff[r] = first float4 of the half
 // row of output r (all equal when UNIFORM, in which case only toff[0] is read).  tbase is passed
 // separately from the offsets so that after inlining the compiler still knows its address space.
+// Operand form: acc_a += (W.re, W.im) * S.x, acc_b += (W.re, W.im) * S.y with the tap PAIR as the
+// packed operand and the folded sample as the scalar one: the tap pair is then the same register
+// pair for up to 2R consecutive FFMA2 (register-reuse cache), which keeps the register-file reads
+// per instruction at <= 2 per bank; the scalar-tap form measured 0.80 of the pipe at best.
 template <int L, int R, bool UNIFORM>
 __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
                                               const float4 *__restrict__ tbase,
@@ -75,13 +76,8 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
 #pragma unroll
     for (int r = 0; r < R; ++r) {                       // centre tap W_0
         const float4 t = tw[UNIFORM ? 0 : r];
-#if PDM_FIR_FORM == 0
-        acc_a[r] = pk_mul_s(t.x, wl[r]);
-        acc_b[r] = pk_mul_s(t.y, wl[r]);
-#else
         acc_a[r] = pk_mul_s(wl[r].x, f4lo(t));
         acc_b[r] = pk_mul_s(wl[r].y, f4lo(t));
-#endif
     }
     float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
 #pragma unroll
@@ -97,16 +93,6 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
 #pragma unroll
             for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r] + k / 2];
         }
-#if PDM_FIR_FORM == 0
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 t = tw[UNIFORM ? 0 : r];
-            const float wre = (k & 1) ? t.z : t.x, wim = (k & 1) ? t.w : t.y;
-            const float2 s = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
-            acc_a[r] = pk_fma_s(wre, s, acc_a[r]);
-            acc_b[r] = pk_fma_s(wim, s, acc_b[r]);
-        }
-#elif PDM_FIR_FORM == 1
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 t = tw[UNIFORM ? 0 : r];
@@ -115,31 +101,6 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
             acc_a[r] = pk_fma_s(s.x, W, acc_a[r]);
             acc_b[r] = pk_fma_s(s.y, W, acc_b[r]);
         }
-#else
-        float2 s[R];
-#pragma unroll
-        for (int r = 0; r < R; ++r) s[r] = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
-#if PDM_FIR_FORM == 2
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 t = tw[UNIFORM ? 0 : r];
-            acc_a[r] = pk_fma_s(s[r].x, (k & 1) ? f4hi(t) : f4lo(t), acc_a[r]);
-        }
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 t = tw[UNIFORM ? 0 : r];
-            acc_b[r] = pk_fma_s(s[r].y, (k & 1) ? f4hi(t) : f4lo(t), acc_b[r]);
-        }
-#else
-#pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float4 t = tw[UNIFORM ? 0 : r];
-            const float2 W = (k & 1) ? f4hi(t) : f4lo(t);
-            acc_a[r] = pk_fma_s(s[r].x, W, acc_a[r]);
-            acc_b[r] = pk_fma_s(s[r].y, W, acc_b[r]);
-        }
-#endif
-#endif
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
@@ -210,7 +171,10 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
             }
             __syncthreads();
         }
-        if (tid < nwarps + 2) prog[tid] = (tid == 0 || tid == nwarps + 1) ? 0x7fffffff : 0;
+        if (tid < nwarps + 2) {                          // sentinels and warps beyond the line: always ahead
+            const bool idle = tid == 0 || tid == nwarps + 1 || (tid - 1) * p.passes * 32 >= p.ngroups;
+            prog[tid] = idle ? 0x7fffffff : 0;
+        }
         {                                                // P(z0): P0[line] or the hand-off
             const float2 *src = (z0 == 0) ? p.P0 + (size_t)line * p.nx : p.handoff + (size_t)slot * p.nx;
             for (int x = tid; x < p.nx; x += T) {
@@ -220,110 +184,106 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
         }
         __syncthreads();
 
-        float2 *cur = buf_a, *nxt = buf_b;
-        float qn[R];
-        {
-            const int g0 = min(warp * p.passes * 32 + lane, p.ngroups - 1);
-            const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)z0 * p.qstride + (size_t)g0 * R);
+        // passes in which this warp has at least one group inside the line (warp-uniform)
+        const int npw = min(p.passes, max(0, (p.ngroups - warp * p.passes * 32 + 31) / 32));
+        if (npw > 0) {
+            float2 *cur = buf_a, *nxt = buf_b;
+            const float4 *const tbase = TAPS_SMEM ? slice : p.half;
+            // A1/A2 run ahead of A3 (neither depends on the wavefield): q is requested two groups
+            // ahead, and the table offsets tn[] / thread-uniformity flag un of the NEXT group are
+            // computed at the top of a group, before the wait on the neighbouring warps.
+            float qn[R];
+            int tn[R];
+            bool un = false;
+            auto load_q = [&](int zq, int pq) {
+                const int gq = min((warp * p.passes + pq) * 32 + lane, p.ngroups - 1);
+                const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)zq * p.qstride + (size_t)gq * R);
 #pragma unroll
-            for (int i = 0; i < R / 4; ++i) {
-                const float4 v = __ldg(qp + i);
-                qn[4 * i] = v.x; qn[4 * i + 1] = v.y; qn[4 * i + 2] = v.z; qn[4 * i + 3] = v.w;
-            }
-        }
-        for (int z = z0; z < z1; ++z) {
-            const bool accumulate = z < wz;
-            for (int pass = 0; pass < p.passes; ++pass) {
-                const int g_raw = (warp * p.passes + pass) * 32 + lane;
-                // whole warp beyond the line: nothing to do in this pass (warp-uniform)
-                const bool warp_active = (warp * p.passes + pass) * 32 < p.ngroups;
-                float qc[R];
+                for (int i = 0; i < R / 4; ++i) {
+                    const float4 v = __ldg(qp + i);
+                    qn[4 * i] = v.x; qn[4 * i + 1] = v.y; qn[4 * i + 2] = v.z; qn[4 * i + 3] = v.w;
+                }
+            };
+            auto index_next = [&]() {
+                int jn[R];
+                bool u = true;
 #pragma unroll
-                for (int r = 0; r < R; ++r) qc[r] = qn[r];
-                {                                        // A1 prefetch: q of the next (z, pass)
-                    int pz = z, pp = pass + 1;
-                    if (pp == p.passes) { pp = 0; ++pz; }
-                    if (pz < z1) {
-                        const int gn = min((warp * p.passes + pp) * 32 + lane, p.ngroups - 1);
-                        const float4 *qp = reinterpret_cast<const float4 *>(
-                            p.q + (size_t)pz * p.qstride + (size_t)gn * R);
+                for (int r = 0; r < R; ++r) {
+                    jn[r] = pdm_index(w, qn[r], ntab_m1);
+                    u = u && (jn[r] == jn[0]);
+                }
+                un = u;
+#pragma unroll
+                for (int r = 0; r < R; ++r) tn[r] = (TAPS_SMEM ? (int)map[jn[r]] : jn[r]) * p.half16;
+            };
+            load_q(z0, 0);
+            index_next();
+            int qz = z0, qp = 1;                         // (z, pass) of the q row requested last
+            if (qp == npw) { qp = 0; ++qz; }
+            if (qz < z1) load_q(qz, qp);
+            for (int z = z0; z < z1; ++z) {
+                const bool accumulate = z < wz;
+                for (int pass = 0; pass < npw; ++pass) {
+                    const int g_raw = (warp * p.passes + pass) * 32 + lane;
+                    const bool active = g_raw < p.ngroups;
+                    const int g = active ? g_raw : p.ngroups - 1;
+                    int toff[R];
+#pragma unroll
+                    for (int r = 0; r < R; ++r) toff[r] = tn[r];
+                    const bool uni = __all_sync(0xffffffffu, un);
+                    index_next();                        // next group's offsets, from the q requested a group ago
+                    if (++qp == npw) { qp = 0; ++qz; }   // A1 prefetch: q two groups ahead
+                    if (qz < z1) load_q(qz, qp);         // else: tn/un of groups that are never run
+                    float4 *prow = reinterpret_cast<float4 *>(my_partial + (size_t)z * p.pstride + (size_t)g * R);
+                    float4 pold[R / 4];
+                    if (accumulate) {                    // A5: old partial row, consumed at the end
+#pragma unroll
+                        for (int i = 0; i < R / 4; ++i) pold[i] = __ldcs(prow + i);
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < R / 4; ++i) pold[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                    }
+                    if (pass == 0 && z > z0) {           // A4: neighbours have completed step z-1
+                        if (lane == 0) {
+                            const int need = z - z0;
+                            while (*(volatile int *)&prog[warp] < need) { }
+                            while (*(volatile int *)&prog[warp + 2] < need) { }
+                            __threadfence_block();
+                        }
+                        __syncwarp();
+                    }
+                    const float2 *base = cur + (HG + g) * GS;
+                    float2 out[R];
+                    if (uni) pdm_fir_group<L, R, true>(base, tbase, toff, out);
+                    else     pdm_fir_group<L, R, false>(base, tbase, toff, out);
+                    if (active) {
+                        const int x0 = g * R;
+                        float2 *dst = nxt + (HG + g) * GS;
+#pragma unroll
+                        for (int i = 0; i < R / 2; ++i) {    // samples beyond nx stay zero (R5)
+                            float2 a = out[2 * i], b = out[2 * i + 1];
+                            if (x0 + 2 * i >= p.nx) a = make_float2(0.f, 0.f);
+                            if (x0 + 2 * i + 1 >= p.nx) b = make_float2(0.f, 0.f);
+                            *reinterpret_cast<float4 *>(dst + 2 * i) = make_float4(a.x, a.y, b.x, b.y);
+                        }
 #pragma unroll
                         for (int i = 0; i < R / 4; ++i) {
-                            const float4 v = __ldg(qp + i);
-                            qn[4 * i] = v.x; qn[4 * i + 1] = v.y; qn[4 * i + 2] = v.z; qn[4 * i + 3] = v.w;
+                            float4 v = pold[i];
+                            v.x += out[4 * i].x; v.y += out[4 * i + 1].x;
+                            v.z += out[4 * i + 2].x; v.w += out[4 * i + 3].x;
+                            __stcs(prow + i, v);
                         }
                     }
                 }
-                if (!warp_active) continue;
-                const bool active = g_raw < p.ngroups;
-                const int g = active ? g_raw : p.ngroups - 1;
-
-                float4 *prow = reinterpret_cast<float4 *>(my_partial + (size_t)z * p.pstride + (size_t)g * R);
-                float4 pold[R / 4];
-                if (accumulate) {                        // A5: old partial row, consumed at the end
-#pragma unroll
-                    for (int i = 0; i < R / 4; ++i) pold[i] = __ldcs(prow + i);
-                } else {
-#pragma unroll
-                    for (int i = 0; i < R / 4; ++i) pold[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+                __syncwarp();                            // A4: publish this warp's step z
+                if (lane == 0) {
+                    __threadfence_block();
+                    *(volatile int *)&prog[warp + 1] = z - z0 + 1;
                 }
-
-                int j[R];
-                bool uni = true;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    j[r] = pdm_index(w, qc[r], ntab_m1);
-                    uni = uni && (j[r] == j[0]);
-                }
-                if (pass == 0 && z > z0) {               // A4: neighbours have completed step z-1
-                    if (lane == 0) {
-                        const int need = z - z0;
-                        while (*(volatile int *)&prog[warp] < need) { }
-                        while (*(volatile int *)&prog[warp + 2] < need) { }
-                        __threadfence_block();
-                    }
-                    __syncwarp();
-                }
-                int toff[R];
-                const float4 *tbase = TAPS_SMEM ? slice : p.half;
-                const float2 *base = cur + (HG + g) * GS;
-                float2 out[R];
-                if (__all_sync(0xffffffffu, uni)) {
-                    toff[0] = (TAPS_SMEM ? (int)map[j[0]] : j[0]) * p.half16;
-#pragma unroll
-                    for (int r = 1; r < R; ++r) toff[r] = toff[0];
-                    pdm_fir_group<L, R, true>(base, tbase, toff, out);
-                } else {
-#pragma unroll
-                    for (int r = 0; r < R; ++r) toff[r] = (TAPS_SMEM ? (int)map[j[r]] : j[r]) * p.half16;
-                    pdm_fir_group<L, R, false>(base, tbase, toff, out);
-                }
-                if (active) {
-                    const int x0 = g * R;
-                    float2 *dst = nxt + (HG + g) * GS;
-#pragma unroll
-                    for (int i = 0; i < R / 2; ++i) {    // samples beyond nx stay zero (R5)
-                        float2 a = out[2 * i], b = out[2 * i + 1];
-                        if (x0 + 2 * i >= p.nx) a = make_float2(0.f, 0.f);
-                        if (x0 + 2 * i + 1 >= p.nx) b = make_float2(0.f, 0.f);
-                        *reinterpret_cast<float4 *>(dst + 2 * i) = make_float4(a.x, a.y, b.x, b.y);
-                    }
-#pragma unroll
-                    for (int i = 0; i < R / 4; ++i) {
-                        float4 v = pold[i];
-                        v.x += out[4 * i].x; v.y += out[4 * i + 1].x;
-                        v.z += out[4 * i + 2].x; v.w += out[4 * i + 3].x;
-                        __stcs(prow + i, v);
-                    }
-                }
+                float2 *t = cur; cur = nxt; nxt = t;
             }
-            __syncwarp();                                // A4: publish this warp's step z
-            if (lane == 0) {
-                __threadfence_block();
-                *(volatile int *)&prog[warp + 1] = z - z0 + 1;
-            }
-            float2 *t = cur; cur = nxt; nxt = t;
         }
+        float2 *const cur = ((z1 - z0) & 1) ? buf_b : buf_a;   // the line at depth z1
         if (z0 == 0) wz = max(wz, z1);                   // a head or a whole line defines rows [0,z1)
         if (z1 < p.nz) {                                 // HEAD: publish the line at depth z1
             __syncthreads();                             // every warp has completed step z1-1
