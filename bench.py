@@ -2,6 +2,7 @@
 """bench.py -- throughput of the f-x poststack depth-migration hot path (BASELINE.json metric).
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 0..3] [--impl ours|reference]
+    python bench.py --sweep [--sweep-taps 15,25,51]     (configs[4], one JSON line per point)
 
 A "step" is one pass of the whole hot path (table look-up, FIR extrapolation, depth marching,
 imaging: SURVEY.md 8(a) A1-A7) over one f-x section: one `pdm_migrate` call.  At N = 1 the
@@ -302,6 +303,69 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         dist.destroy_process_group()
 
 
+# ------------------------------------------------------------------------------- configs[4] sweep
+SWEEP_NX = (1024, 4096, 16384, 32768)
+SWEEP_NW = (64, 256, 1024, 2048)
+SWEEP_TAPS = (15, 25, 51)
+
+
+def run_sweep(args):
+    """BASELINE.json configs[4]: samples/s and roofline fraction per (nx, nw, taps) point, one JSON
+    line each (parity of sampled points is tests/test_gpu_parity.py's job, not this loop's)."""
+    import torch
+
+    import paper_1912_05529_b200 as pdm
+    from pdm_inputs.configs import sweep_point
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    pdm.load_library()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    with open("/root/repo/MEASURED_PEAKS.json") if os.path.exists("/root/repo/MEASURED_PEAKS.json") \
+            else open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+        hbm_gbs = json.load(f)["hbm_gbs"]
+    only = {int(t) for t in args.sweep_taps.split(",")} if args.sweep_taps else set(SWEEP_TAPS)
+    for ntaps in SWEEP_TAPS:
+        if ntaps not in only:
+            continue
+        for nx in SWEEP_NX:
+            for nw in SWEEP_NW:
+                cfg = sweep_point(nx, nw, ntaps)
+                plan = pdm.Plan.from_config(cfg, args.flags)
+                info = plan.info
+                P0 = torch.from_numpy(cfg["P0"]).to(dev)
+                image = torch.empty((cfg["nz"], nx), dtype=torch.float32, device=dev)
+                steps = int(max(2, min(args.steps, 4e10 // info["samples"])))
+                for _ in range(3):
+                    plan.migrate(P0, image, stream=stream)
+                torch.cuda.synchronize(dev)
+                ms = []
+                for _ in range(steps):
+                    flush.zero_()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    plan.migrate(P0, image, stream=stream)
+                    b.record(stream)
+                    torch.cuda.synchronize(dev)
+                    ms.append(a.elapsed_time(b))
+                t = float(np.median(ms)) * 1e-3
+                sps = info["samples"] / t
+                tiled = info["path"] == pdm.PDM_PATH_TILED
+                out = {"workload": f"configs[4] nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps}",
+                       "path": {1: "smem-marching", 2: "x-tiled", 3: "naive"}.get(info["path"]),
+                       "taps_mode": info["taps_mode"], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
+                       "launches": info["launches_per_migrate"], "steps": steps, "ms": t * 1e3,
+                       "samples_per_s": sps,
+                       "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                       "frac_hbm_16B_per_sample": (sps * 16 / (hbm_gbs * 1e9)) if tiled else None}
+                print(json.dumps(out), flush=True)
+                plan.close()
+                del P0, image
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -311,11 +375,16 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--flags", type=lambda s: int(s, 0), default=0, help="pdm_create flags word")
     ap.add_argument("--cpu-lines-per-thread", type=int, default=16)
+    ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep, one JSON line per point")
+    ap.add_argument("--sweep-taps", default="", help="comma list of tap counts to sweep (default 15,25,51)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.impl == "reference":
+    if args.sweep:
+        if rank == 0:
+            run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     else:
         run_ours(args, rank, local_rank, world)

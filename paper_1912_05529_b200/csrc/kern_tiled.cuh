@@ -1,11 +1,16 @@
 // kern_tiled.cuh -- PDM_PATH_TILED: x-tiled per-depth-step kernel with
 // +-L halos for lines too long for shared memory (BASELINE.json configs[4], nx = 32768).
 // Closest to what the paper itself did (planes in global memory, one grid-wide
-// synchronisation per depth level), but: the tile + halo is staged once in shared memory, the
-// arithmetic is the same register-tiled folded FIR as the main path (pdm_fir_group), a CTA
-// walks a GROUP of frequencies for its x-tile so the q tile is read once and Re P is summed
-// over the group in registers in fixed order (the paper's K2 disappears), and planes ping-pong
-// in HBM: 8 B read + 8 B written per sample (+ halo 2*HG*R/tile_x).
+// synchronisation per depth level = one launch per level), but:
+//   * one resident wave of CTAs per launch; a CTA owns an x-tile and walks a GROUP of frequencies,
+//     so the q tile is read once and Re P is summed over the group in registers in fixed order
+//     (the paper's K2 disappears into a small fixed-order reduction over the groups);
+//   * the tile + halo of the NEXT frequency is copied global -> shared memory with cp.async while
+//     the current one is computed (double buffer), zero-filled outside [0,nx) (R5);
+//   * the arithmetic is the same register-tiled folded FIR as the main path (pdm_fir_group);
+//   * results go through a shared-memory tile so that the plane is written in full 512-byte
+//     warp transactions.
+// HBM traffic: 8 B read + 8 B written per sample (+ halo 2*HG*R/tile_x), planes ping-pong.
 #pragma once
 #include "pdm_common.cuh"
 #include "kern_march.cuh"
@@ -24,20 +29,49 @@ struct pdm_tiled_params {
     int z, w_per_group;
 };
 
-template <int L, int R>
+// CH = samples per async-copy chunk: 2 (16-byte copies; needs nx even and 16-byte aligned planes)
+// or 1 (8-byte copies, any nx).
+template <int CH>
+__device__ __forceinline__ void pdm_cp_async(float2 *dst_smem, const float2 *src, bool valid)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+    const unsigned n = valid ? 8u * CH : 0u;              // src-size 0: the chunk is zero-filled
+    if (CH == 2) asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
+    else         asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
+}
+
+template <int L, int R, int CH>
 __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm_tiled_params p)
 {
     constexpr int HG = pdm_halo_groups<L, R>();
     constexpr int GS = R + 2;
+    constexpr int T = PDM_TILED_THREADS;
+    constexpr int IN_SLOTS = (T + 2 * HG) * GS;
     extern __shared__ __align__(16) unsigned char pdm_smem[];
-    float2 *line = reinterpret_cast<float2 *>(pdm_smem);
+    float2 *ibuf = reinterpret_cast<float2 *>(pdm_smem);          // [2][IN_SLOTS]
+    float2 *obuf = ibuf + 2 * IN_SLOTS;                           // [T * GS]
 
-    const int tid = threadIdx.x, T = blockDim.x;
+    const int tid = threadIdx.x;
     const int tile_x0 = blockIdx.x * T * R;
     const int x0 = tile_x0 + tid * R;
     const int ntab_m1 = p.ntab - 1;
     const int w_begin = blockIdx.y * p.w_per_group;
     const int w_end = min(p.nw, w_begin + p.w_per_group);
+
+    auto issue_load = [&](int iw, int b) {
+        const float2 *src = p.Pin + (size_t)iw * p.nx;
+        float2 *dst = ibuf + b * IN_SLOTS;
+        constexpr int NCH = (T + 2 * HG) * R / CH;
+        for (int c = tid; c < NCH; c += T) {
+            const int s = c * CH, g = s / R;
+            const int x = tile_x0 - HG * R + s;
+            const bool valid = x >= 0 && x < p.nx;             // CH == 2: x and nx are even
+            pdm_cp_async<CH>(dst + g * GS + (s - g * R), src + (valid ? x : 0), valid);
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    if (w_begin < w_end) issue_load(w_begin, 0);
 
     float qc[R];
     {
@@ -53,19 +87,18 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
 #pragma unroll
     for (int r = 0; r < R; ++r) img[r] = 0.f;
 
-    const int nload = (T + 2 * HG) * R;                  // samples of tile + both halos
-    for (int iw = w_begin; iw < w_end; ++iw) {
+    for (int iw = w_begin, it = 0; iw < w_end; ++iw, ++it) {
+        const int b = it & 1;
         const float w = p.omega[iw];
-        const float2 *src = p.Pin + (size_t)iw * p.nx;
-        __syncthreads();                                  // previous frequency finished reading
-        for (int s = tid; s < nload; s += T) {
-            const int x = tile_x0 - HG * R + s;
-            const int g = s / R;
-            float2 v = make_float2(0.f, 0.f);             // R5: zero outside [0,nx)
-            if (x >= 0 && x < p.nx) v = src[x];
-            line[g * GS + (s - g * R)] = v;
+        // all threads are past the compute of iteration it-1 (barrier before its copy-out), so the
+        // buffer it read, b^1, may be refilled now
+        if (iw + 1 < w_end) {
+            issue_load(iw + 1, b ^ 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
-        __syncthreads();
+        __syncthreads();                                   // tile of iw complete; obuf of it-1 drained
 
         int j[R], toff[R];
         bool uni = true;
@@ -76,22 +109,36 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) toff[r] = j[r] * p.half16;
-        const float2 *base = line + (HG + tid) * GS;
+        const float2 *base = ibuf + b * IN_SLOTS + (HG + tid) * GS;
         float2 out[R];
         if (__all_sync(0xffffffffu, uni)) pdm_fir_group<L, R, true>(base, p.half, toff, out);
         else                              pdm_fir_group<L, R, false>(base, p.half, toff, out);
 
-        float2 *dst = p.Pout + (size_t)iw * p.nx;
+        float2 *od = obuf + tid * GS;
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            if (x0 + r < p.nx) dst[x0 + r] = out[r];
-            img[r] += out[r].x;                           // A5: fixed (increasing w) order
+        for (int i = 0; i < R / 2; ++i)
+            *reinterpret_cast<float4 *>(od + 2 * i) = make_float4(out[2 * i].x, out[2 * i].y, out[2 * i + 1].x, out[2 * i + 1].y);
+#pragma unroll
+        for (int r = 0; r < R; ++r) img[r] += out[r].x;   // A5: fixed (increasing w) order
+        __syncthreads();                                   // obuf complete; ibuf[b] no longer read
+
+        float2 *dst = p.Pout + (size_t)iw * p.nx;
+        constexpr int NCH = T * R / CH;
+#pragma unroll
+        for (int c = tid; c < NCH; c += T) {               // full-width warp stores
+            const int s = c * CH, g = s / R;
+            const int x = tile_x0 + s;
+            if (x < p.nx) {
+                const float2 *sp = obuf + g * GS + (s - g * R);
+                if (CH == 2) *reinterpret_cast<float4 *>(dst + x) = *reinterpret_cast<const float4 *>(sp);
+                else         dst[x] = *sp;
+            }
         }
     }
-    if (x0 < p.pstride) {
+    if (w_begin < w_end && x0 < p.pstride) {
         float *prow = p.partial + ((size_t)blockIdx.y * p.nz + p.z) * p.pstride + x0;
 #pragma unroll
-        for (int r = 0; r < R; ++r)
-            if (x0 + r < p.pstride) prow[r] = img[r];
+        for (int i = 0; i < R / 4; ++i)
+            *reinterpret_cast<float4 *>(prow + 4 * i) = make_float4(img[4 * i], img[4 * i + 1], img[4 * i + 2], img[4 * i + 3]);
     }
 }

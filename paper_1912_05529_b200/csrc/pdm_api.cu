@@ -153,10 +153,10 @@ static march_fn march_kernel_for(int L, bool taps_smem)
     default: return nullptr;
     }
 }
-static tiled_fn tiled_kernel_for(int L)
+static tiled_fn tiled_kernel_for(int L, bool wide)
 {
     switch (L) {
-#define X(LL) case LL: return pdm_tiled_step<LL, PDM_R>;
+#define X(LL) case LL: return wide ? pdm_tiled_step<LL, PDM_R, 2> : pdm_tiled_step<LL, PDM_R, 1>;
         PDM_FOR_EACH_L(X)
 #undef X
     default: return nullptr;
@@ -298,7 +298,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
 
     if (want == PDM_PATH_CLUSTER) return PDM_ERR_UNSUPPORTED;       // not built in this round
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
-    if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;
+    if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;  // (tiled_kernel_for has the same L list)
     if (want == PDM_PATH_AUTO) p->path = lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE);
     else p->path = (int)want;
 
@@ -359,18 +359,26 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->threads = PDM_TILED_THREADS;
         p->tile_x = PDM_TILED_THREADS * R;
         const int xtiles = (nx + p->tile_x - 1) / p->tile_x;
-        int wgroups = std::max(1, std::min(nw, (4 * p->sm_count + xtiles - 1) / xtiles));
+        // double-buffered input tile (+ halos) and one output tile
+        p->smem_bytes = (3 * PDM_TILED_THREADS + 4 * HG) * (R + 2) * (int)sizeof(float2);
+        int per_sm = 0;
+        for (int wide = 0; wide < 2; ++wide) {
+            tiled_fn fn = tiled_kernel_for(L, wide != 0);
+            PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             p->smem_bytes));
+            PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn,
+                                                                      PDM_TILED_THREADS, (size_t)p->smem_bytes));
+        }
+        if (per_sm < 1) return PDM_ERR_UNSUPPORTED;
+        p->ctas_per_sm = per_sm;
+        // ONE resident wave per depth step: x-tiles x frequency groups <= SMs x CTAs per SM
+        int wgroups = std::max(1, std::min(nw, p->sm_count * per_sm / xtiles));
         const int wpg = (nw + wgroups - 1) / wgroups;
         wgroups = (nw + wpg - 1) / wpg;
         p->wgroups = wgroups;
         p->grid = xtiles * wgroups;
-        p->ctas_per_sm = 2;
-        p->smem_bytes = (PDM_TILED_THREADS + 2 * HG) * (R + 2) * (int)sizeof(float2);
         p->launches = nz + 1;
         p->n_partial = wgroups;
-        tiled_fn fn = tiled_kernel_for(L);
-        PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         p->smem_bytes));
         if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)wgroups * nz * p->qstride)) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_plane[0], (size_t)nw * nx)) != PDM_OK) return rc;
@@ -432,7 +440,9 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
         a.qstride = p->qstride; a.pstride = p->qstride; a.half16 = p->half16;
         a.w_per_group = (nw + p->wgroups - 1) / p->wgroups;
-        tiled_fn fn = tiled_kernel_for(L);
+        // 16-byte async copies need every plane row 16-byte aligned: nx even and an aligned P0
+        const bool wide = (nx % 2 == 0) && (((uintptr_t)P0_dev & 15u) == 0);
+        tiled_fn fn = tiled_kernel_for(L, wide);
         dim3 grid((nx + p->tile_x - 1) / p->tile_x, p->wgroups);
         const float2 *src = P0;
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
