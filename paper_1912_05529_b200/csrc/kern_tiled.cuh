@@ -5,8 +5,11 @@
 //   * one resident wave of CTAs per launch; a CTA owns an x-tile and walks a GROUP of frequencies,
 //     so the q tile is read once and Re P is summed over the group in registers in fixed order
 //     (the paper's K2 disappears into a small fixed-order reduction over the groups);
-//   * the tile + halo of the NEXT frequency is copied global -> shared memory with cp.async while
-//     the current one is computed (double buffer), zero-filled outside [0,nx) (R5);
+//   * every WARP runs its own pipeline over its 32 x R samples of the tile: the sub-tile + halo of
+//     the NEXT frequency is copied global -> shared memory with cp.async while the current one is
+//     computed (double buffer per warp), zero-filled outside [0,nx) (R5); only __syncwarp inside
+//     the frequency loop, so the 16 warps of an SM drift apart and loads, FMAs and stores overlap
+//     (halo groups are fetched by both neighbouring warps: L2 hits, not HBM traffic);
 //   * the arithmetic is the same register-tiled folded FIR as the main path (pdm_fir_group);
 //   * results go through a shared-memory tile so that the plane is written in full 512-byte
 //     warp transactions.
@@ -46,14 +49,15 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
     constexpr int HG = pdm_halo_groups<L, R>();
     constexpr int GS = R + 2;
     constexpr int T = PDM_TILED_THREADS;
-    constexpr int IN_SLOTS = (T + 2 * HG) * GS;
+    constexpr int IN_SLOTS = (32 + 2 * HG) * GS;                  // per warp and buffer
+    constexpr int WARP_SLOTS = 2 * IN_SLOTS + 32 * GS;            // two input buffers + output tile
     extern __shared__ __align__(16) unsigned char pdm_smem[];
-    float2 *ibuf = reinterpret_cast<float2 *>(pdm_smem);          // [2][IN_SLOTS]
-    float2 *obuf = ibuf + 2 * IN_SLOTS;                           // [T * GS]
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    float2 *ibuf = reinterpret_cast<float2 *>(pdm_smem) + warp * WARP_SLOTS;   // [2][IN_SLOTS]
+    float2 *obuf = ibuf + 2 * IN_SLOTS;                                        // [32 * GS]
 
-    const int tid = threadIdx.x;
-    const int tile_x0 = blockIdx.x * T * R;
-    const int x0 = tile_x0 + tid * R;
+    const int tile_x0 = blockIdx.x * T * R + warp * 32 * R;       // this warp's first sample
+    const int x0 = tile_x0 + lane * R;
     const int ntab_m1 = p.ntab - 1;
     const int w_begin = blockIdx.y * p.w_per_group;
     const int w_end = min(p.nw, w_begin + p.w_per_group);
@@ -61,8 +65,8 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
     auto issue_load = [&](int iw, int b) {
         const float2 *src = p.Pin + (size_t)iw * p.nx;
         float2 *dst = ibuf + b * IN_SLOTS;
-        constexpr int NCH = (T + 2 * HG) * R / CH;
-        for (int c = tid; c < NCH; c += T) {
+        constexpr int NCH = (32 + 2 * HG) * R / CH;
+        for (int c = lane; c < NCH; c += 32) {
             const int s = c * CH, g = s / R;
             const int x = tile_x0 - HG * R + s;
             const bool valid = x >= 0 && x < p.nx;             // CH == 2: x and nx are even
@@ -90,7 +94,7 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
     for (int iw = w_begin, it = 0; iw < w_end; ++iw, ++it) {
         const int b = it & 1;
         const float w = p.omega[iw];
-        // all threads are past the compute of iteration it-1 (barrier before its copy-out), so the
+        // the warp is past the compute of iteration it-1 (__syncwarp before its copy-out), so the
         // buffer it read, b^1, may be refilled now
         if (iw + 1 < w_end) {
             issue_load(iw + 1, b ^ 1);
@@ -98,7 +102,7 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         } else {
             asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
-        __syncthreads();                                   // tile of iw complete; obuf of it-1 drained
+        __syncwarp();                                      // tile of iw complete; obuf of it-1 drained
 
         int j[R], toff[R];
         bool uni = true;
@@ -109,23 +113,23 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) toff[r] = j[r] * p.half16;
-        const float2 *base = ibuf + b * IN_SLOTS + (HG + tid) * GS;
+        const float2 *base = ibuf + b * IN_SLOTS + (HG + lane) * GS;
         float2 out[R];
         if (__all_sync(0xffffffffu, uni)) pdm_fir_group<L, R, true>(base, p.half, toff, out);
         else                              pdm_fir_group<L, R, false>(base, p.half, toff, out);
 
-        float2 *od = obuf + tid * GS;
+        float2 *od = obuf + lane * GS;
 #pragma unroll
         for (int i = 0; i < R / 2; ++i)
             *reinterpret_cast<float4 *>(od + 2 * i) = make_float4(out[2 * i].x, out[2 * i].y, out[2 * i + 1].x, out[2 * i + 1].y);
 #pragma unroll
         for (int r = 0; r < R; ++r) img[r] += out[r].x;   // A5: fixed (increasing w) order
-        __syncthreads();                                   // obuf complete; ibuf[b] no longer read
+        __syncwarp();                                      // obuf complete; ibuf[b] no longer read
 
         float2 *dst = p.Pout + (size_t)iw * p.nx;
-        constexpr int NCH = T * R / CH;
+        constexpr int NCH = 32 * R / CH;
 #pragma unroll
-        for (int c = tid; c < NCH; c += T) {               // full-width warp stores
+        for (int c = lane; c < NCH; c += 32) {             // full-width warp stores
             const int s = c * CH, g = s / R;
             const int x = tile_x0 + s;
             if (x < p.nx) {

@@ -359,8 +359,8 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->threads = PDM_TILED_THREADS;
         p->tile_x = PDM_TILED_THREADS * R;
         const int xtiles = (nx + p->tile_x - 1) / p->tile_x;
-        // double-buffered input tile (+ halos) and one output tile
-        p->smem_bytes = (3 * PDM_TILED_THREADS + 4 * HG) * (R + 2) * (int)sizeof(float2);
+        // per warp: double-buffered input sub-tile (+ halos) and one output sub-tile
+        p->smem_bytes = (PDM_TILED_THREADS / 32) * (2 * (32 + 2 * HG) + 32) * (R + 2) * (int)sizeof(float2);
         int per_sm = 0;
         for (int wide = 0; wide < 2; ++wide) {
             tiled_fn fn = tiled_kernel_for(L, wide != 0);
