@@ -327,13 +327,12 @@ def run_sweep(args):
     with open("/root/repo/MEASURED_PEAKS.json") if os.path.exists("/root/repo/MEASURED_PEAKS.json") \
             else open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
         hbm_gbs = json.load(f)["hbm_gbs"]
-    only = {int(t) for t in args.sweep_taps.split(",")} if args.sweep_taps else set(SWEEP_TAPS)
-    for ntaps in SWEEP_TAPS:
-        if ntaps not in only:
-            continue
-        for nx in SWEEP_NX:
-            for nw in SWEEP_NW:
-                cfg = sweep_point(nx, nw, ntaps)
+    def pick(arg, full):
+        return tuple(int(t) for t in arg.split(",")) if arg else full
+    for ntaps in pick(args.sweep_taps, SWEEP_TAPS):
+        for nx in pick(args.sweep_nx, SWEEP_NX):
+            for nw in pick(args.sweep_nw, SWEEP_NW):
+                cfg = sweep_point(nx, nw, ntaps, model=args.sweep_model)
                 plan = pdm.Plan.from_config(cfg, args.flags)
                 info = plan.info
                 P0 = torch.from_numpy(cfg["P0"]).to(dev)
@@ -354,7 +353,7 @@ def run_sweep(args):
                 t = float(np.median(ms)) * 1e-3
                 sps = info["samples"] / t
                 tiled = info["path"] == pdm.PDM_PATH_TILED
-                out = {"workload": f"configs[4] nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps}",
+                out = {"workload": f"configs[4] nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} velocity={args.sweep_model}",
                        "path": {1: "smem-marching", 2: "x-tiled", 3: "naive"}.get(info["path"]),
                        "taps_mode": info["taps_mode"], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                        "launches": info["launches_per_migrate"], "steps": steps, "ms": t * 1e3,
@@ -377,6 +376,11 @@ def main():
     ap.add_argument("--cpu-lines-per-thread", type=int, default=16)
     ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep, one JSON line per point")
     ap.add_argument("--sweep-taps", default="", help="comma list of tap counts to sweep (default 15,25,51)")
+    ap.add_argument("--sweep-nx", default="", help="comma list of nx (default 1024,4096,16384,32768)")
+    ap.add_argument("--sweep-nw", default="", help="comma list of nw (default 64,256,1024,2048)")
+    ap.add_argument("--sweep-model", default="field", choices=["field", "layers"],
+                    help="velocity of the sweep: BASELINE.json's random field, or flat layers "
+                         "(warp-uniform table rows: the HBM-bound regime of the x-tiled path)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))

@@ -324,17 +324,23 @@ SWEEP_NW = (64, 256, 1024, 2048)
 SWEEP_TAPS = (15, 25, 51)
 
 
-def sweep_point(nx: int, nw: int, ntaps: int, nz: int = 256, seed: int = BASE_SEED + 4):
-    """One point of the configs[4] throughput sweep (random-field velocity, Gaussian P0)."""
+def sweep_point(nx: int, nw: int, ntaps: int, nz: int = 256, seed: int = BASE_SEED + 4,
+                model: str = "field"):
+    """One point of the configs[4] throughput sweep (random-field velocity, Gaussian P0).
+    model="layers" swaps in 6 flat layers (1500-5000 m/s): the same sizes with warp-uniform table
+    rows, the regime where the x-tiled path is bound by HBM rather than by the tap gather."""
     dx = dz = 10.0
     rng = np.random.default_rng([seed, nx])
-    v = random_field_velocity(rng, nz, nx, dz, dx)
+    if model == "layers":
+        v, _ = layered_velocity(rng, nz, nx, 6, 1500.0, 5000.0)
+    else:
+        v = random_field_velocity(rng, nz, nx, dz, dx)
     omega = (2.0 * np.pi * np.linspace(3.0, 60.0, nw)).astype(np.float32)
     rng2 = np.random.default_rng([seed, nx, nw])
     P0 = np.empty((nw, nx), dtype=np.complex64)
     P0.real = rng2.standard_normal((nw, nx), dtype=np.float32)
     P0.imag = rng2.standard_normal((nw, nx), dtype=np.float32)
-    return _finish(f"configs[4] nx={nx} nw={nw} taps={ntaps}", nx, nz, dx, dz, ntaps, omega, v, P0)
+    return _finish(f"configs[4] nx={nx} nw={nw} taps={ntaps} model={model}", nx, nz, dx, dz, ntaps, omega, v, P0)
 
 
 def make_config(k: int, seed: int | None = None):

@@ -122,6 +122,49 @@ def test_depth_split_balancing_matches_oracle_and_whole_line_schedule(pdm, nx, n
         assert torch.equal(a, b) and np.array_equal(a.cpu().numpy(), img_b)
 
 
+@pytest.mark.parametrize("nx,warps,ntaps,model", [
+    (3000, 2, 25, "layers"),     # 375 groups on 2 warps: 6 passes per warp, ragged last pass
+    (1000, 3, 15, "field"),      # 125 groups on 3 warps: the last warp is partly idle
+    (700, 12, 7, "white"),       # 88 groups on 12 warps: warps 3..11 idle (always-ahead flags)
+])
+def test_neighbour_flag_marching_with_forced_thread_counts(pdm, nx, warps, ntaps, model):
+    """The marching kernel synchronises depth steps with per-warp progress flags between
+    neighbouring warps (no CTA barrier); force odd warp/pass layouts and check parity and
+    bit-identical repeats."""
+    import torch
+    cfg = pdm_inputs.random_problem(23, nx, 40, 5, ntaps, model=model)
+    flags = pdm.PDM_PATH_SMEM | (warps << pdm.PDM_THREADS_SHIFT)
+    ref = oracle.migrate(cfg)
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        assert plan.info["threads_per_cta"] == 32 * warps
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(p0).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    rel, mx = errors(a.cpu().numpy(), ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+
+
+def test_tiled_path_with_unaligned_plane_pointer(pdm):
+    """Even nx but a P0 that is only 8-byte aligned: the tiled kernel must take its 8-byte
+    async-copy variant and still match the 16-byte one bit for bit."""
+    import torch
+    cfg = pdm_inputs.random_problem(29, 2600, 12, 6, 25, model="field")
+    with pdm.Plan.from_config(cfg, pdm.PDM_PATH_TILED) as plan:
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        store = torch.empty(p0.numel() + 1, dtype=p0.dtype, device="cuda")
+        shifted = store[1:].view(p0.shape)
+        shifted.copy_(p0)
+        assert shifted.data_ptr() % 16 == 8
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(shifted).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    rel, mx = errors(a.cpu().numpy(), oracle.migrate(cfg))
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+
+
 # ---------------------------------------------------------------- BASELINE.json configs
 def test_config0_all_paths(pdm, config0):
     ref = oracle.migrate(config0)
