@@ -39,6 +39,10 @@ UNIT = "samples/s"
 # lanes x 2 flop/FMA x 1.965 GHz max SM clock.  The FFMA-chain microbenchmark (pdm_fp32_peak)
 # reads 71-73 TFLOP/s on this pool; both are reported.
 FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
+# committed `ncu --set full` capture of this command (profiles/r01_march_config3.md, section 2):
+# 27.23 GB + 29.55 GB on configs[3] (the per-CTA partial-image read-modify-write).
+NCU_DRAM_BYTES_PER_LAUNCH = {3: 27.230737e9 + 29.551742e9}
 
 
 def load_workload(k: int, rank: int, world: int) -> dict:
@@ -265,7 +269,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
                     "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                     "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
-                    "traffic": None,
+                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if world == 1 and not args.flags else None,
+                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01_march_config3.md)",
                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                    "MEASURED_PEAKS.json has no FP32 entry",
                     "ffma_chain_measured_tflops": fma_peak,
