@@ -370,6 +370,51 @@ def run_sweep(args):
                 del P0, image
 
 
+# ------------------------------------------------------------------------------- t -> f transform
+def run_tf(args):
+    """the time -> frequency transform of the input section at configs[3]'s size
+    (nt = 4096 samples, nx = 6144 traces, the 803 bins of 2-100 Hz), one JSON line."""
+    import torch
+
+    import paper_1912_05529_b200 as pdm
+    from pdm_inputs.configs import dft_bin_omegas
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    pdm.load_library()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream(dev)
+    nt, dt, nx = 4096, 0.002, 6144
+    omega = dft_bin_omegas(nt, dt, 2.0, 100.0)
+    bins = np.rint(np.asarray(omega, np.float64) * nt * dt / (2 * np.pi)).astype(np.int32)
+    section = torch.randn((nt, nx), dtype=torch.float32, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    with pdm.SectionTransform(nt, nx, bins) as tf:
+        out = tf.forward(section)
+        for _ in range(max(args.warmup, 3)):
+            tf.forward(section, out=out, stream=stream)
+        torch.cuda.synchronize(dev)
+        ms = []
+        for _ in range(args.steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            tf.forward(section, out=out, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize(dev)
+            ms.append(a.elapsed_time(b))
+    t = float(np.median(ms)) * 1e-3
+    flops = 4.0 * nt * bins.size * nx                     # 2 FMAs per (bin, time sample, trace)
+    print(json.dumps({"workload": f"t->f transform nt={nt} nx={nx} nw={bins.size} (configs[3] record)",
+                      "kernel": "pdm_tf_kernel", "steps": args.steps, "ms": t * 1e3,
+                      "bin_trace_outputs_per_s": bins.size * nx / t,
+                      "roofline": {"bound": "alu", "achieved": flops / t / 1e12,
+                                   "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
+                                   "frac": flops / t / 1e12 / FP32_PEAK_NOMINAL_TFLOPS},
+                      "share_of_migration": "compare ms with bench.py's ms_per_step on configs[3]"}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -379,6 +424,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--flags", type=lambda s: int(s, 0), default=0, help="pdm_create flags word")
     ap.add_argument("--cpu-lines-per-thread", type=int, default=16)
+    ap.add_argument("--tf", action="store_true", help="time the t->f transform of the section (SURVEY 8(f) N1)")
     ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep, one JSON line per point")
     ap.add_argument("--sweep-taps", default="", help="comma list of tap counts to sweep (default 15,25,51)")
     ap.add_argument("--sweep-nx", default="", help="comma list of nx (default 1024,4096,16384,32768)")
@@ -390,7 +436,10 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
-    if args.sweep:
+    if args.tf:
+        if rank == 0:
+            run_tf(args)
+    elif args.sweep:
         if rank == 0:
             run_sweep(args)
     elif args.impl == "reference":

@@ -164,6 +164,31 @@ int pdm_debug_table_index(const float *omega, const float *velocity, int n,
  */
 int pdm_fp32_peak(int packed, int iters, int repeats, void *cuda_stream, double *tflops_out);
 
+/*
+ * ---- time -> frequency transform of the input section ----------------------
+ * PAPER.md:51, Alg. 1 (:58): every trace of the zero-offset section is Fourier transformed along
+ * the TIME axis only; the depth loop consumes the resulting f-x section.  For the
+ * nw selected DFT bins (omega_j = 2*pi*bins[j] / (nt*dt)) this computes, in FP32,
+ *
+ *     P0[j][x] = sum_{n=0}^{nt-1} section[n][x] * exp(-2*pi*i * bins[j] * n / nt)     (no scaling)
+ *
+ * i.e. exactly the layout pdm_migrate reads.  Twiddles come from an nt-entry table built in double
+ * at create time and indexed by the exact integer (bins[j]*n) mod nt.
+ *
+ * pdm_tf_create  -- bins: HOST int[nw], each in [0, nt/2]; copies what it needs.
+ *                   Errors: PDM_ERR_INVALID_ARG (NULL, sizes <= 0, bin out of range),
+ *                   PDM_ERR_UNSUPPORTED (no CC 10.x device, nt > PDM_TF_MAX_NT), PDM_ERR_NOMEM/CUDA.
+ * pdm_tf_forward -- section_dev: DEVICE float[nt][nx] (time-major, x fastest), read-only;
+ *                   P0_dev: DEVICE pdm_c64[nw][nx], overwritten.  Enqueue only on cuda_stream
+ *                   (no allocation, no host sync, no copies); deterministic.
+ * pdm_tf_destroy -- frees the plan; NULL is allowed.
+ */
+typedef struct pdm_tf pdm_tf;
+#define PDM_TF_MAX_NT 8192         /* the twiddle table (8 B per entry) lives in shared memory */
+int pdm_tf_create(pdm_tf **out, int nt, int nx, int nw, const int *bins);
+int pdm_tf_forward(pdm_tf *tf, const float *section_dev, pdm_c64 *P0_dev, void *cuda_stream);
+int pdm_tf_destroy(pdm_tf *tf);
+
 #ifdef __cplusplus
 }
 #endif

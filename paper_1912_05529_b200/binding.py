@@ -29,7 +29,8 @@ PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TILE_SHIFT = 8, 16, 20
 
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
-                    "pdm_profile_enable", "pdm_profile_read")
+                    "pdm_profile_enable", "pdm_profile_read",
+                    "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy")
 
 
 class PdmInfo(ctypes.Structure):
@@ -84,6 +85,12 @@ def load_library(path: str | None = None):
     lib.pdm_profile_enable.argtypes = [vp, ci]
     lib.pdm_profile_read.restype = ci
     lib.pdm_profile_read.argtypes = [vp, ctypes.POINTER(cf), ctypes.POINTER(cf)]
+    lib.pdm_tf_create.restype = ci
+    lib.pdm_tf_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, vp]
+    lib.pdm_tf_forward.restype = ci
+    lib.pdm_tf_forward.argtypes = [vp, vp, vp, vp]
+    lib.pdm_tf_destroy.restype = ci
+    lib.pdm_tf_destroy.argtypes = [vp]
     _lib = lib
     return lib
 
@@ -169,6 +176,62 @@ def pdm_fp32_peak(packed: bool = True, iters: int = 20000, repeats: int = 5, cud
     if rc != PDM_OK:
         raise PdmError(rc, "pdm_fp32_peak")
     return float(val.value)
+
+
+def pdm_tf_create(nt: int, nx: int, nw: int, bins):
+    """-> (rc, handle or None).  bins: int32 array [nw] of DFT bins in [0, nt/2] (host)."""
+    b = np.ascontiguousarray(bins, dtype=np.int32)
+    h = ctypes.c_void_p()
+    rc = load_library().pdm_tf_create(ctypes.byref(h), int(nt), int(nx), int(nw),
+                                      b.ctypes.data_as(ctypes.c_void_p) if b.size else None)
+    return rc, (h if rc == PDM_OK else None)
+
+
+def pdm_tf_forward(handle, section_ptr: int, P0_ptr: int, cuda_stream: int = 0) -> int:
+    return load_library().pdm_tf_forward(handle, ctypes.c_void_p(section_ptr), ctypes.c_void_p(P0_ptr),
+                                         ctypes.c_void_p(cuda_stream))
+
+
+def pdm_tf_destroy(handle) -> int:
+    return load_library().pdm_tf_destroy(handle)
+
+
+class SectionTransform:
+    """Owns a pdm_tf: time-major section float32 [nt][nx] (cuda) -> P0 complex64 [nw][nx] (cuda)."""
+
+    def __init__(self, nt: int, nx: int, bins):
+        self.nt, self.nx = int(nt), int(nx)
+        self.bins = np.ascontiguousarray(bins, dtype=np.int32)
+        rc, self._h = pdm_tf_create(self.nt, self.nx, self.bins.size, self.bins)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_tf_create")
+
+    def forward(self, section, out=None, stream=None):
+        import torch
+        if not (section.is_cuda and section.dtype == torch.float32 and section.is_contiguous()
+                and tuple(section.shape) == (self.nt, self.nx)):
+            raise ValueError("section must be a contiguous cuda float32 tensor [nt][nx]")
+        if out is None:
+            out = torch.empty((self.bins.size, self.nx), dtype=torch.complex64, device=section.device)
+        elif not (out.is_cuda and out.dtype == torch.complex64 and out.is_contiguous()
+                  and tuple(out.shape) == (self.bins.size, self.nx)):
+            raise ValueError("out must be a contiguous cuda complex64 tensor [nw][nx]")
+        st = (stream or torch.cuda.current_stream(section.device)).cuda_stream
+        rc = pdm_tf_forward(self._h, section.data_ptr(), out.data_ptr(), st)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_tf_forward")
+        return out
+
+    def close(self):
+        if self._h is not None:
+            pdm_tf_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
 
 
 # ------------------------------------------------------------------ convenience wrapper

@@ -595,3 +595,97 @@ extern "C" int pdm_fp32_peak(int packed, int iters, int repeats, void *cuda_stre
     *tflops_out = flops / (best_ms * 1e-3) / 1e12;
     return PDM_OK;
 }
+
+// ------------------------------------------------------------------------------------------------
+// time -> frequency transform of the input section
+// ------------------------------------------------------------------------------------------------
+#include "kern_tf.cuh"
+
+struct pdm_tf {
+    int nt, nx, nw, device, smem_bytes, warps;
+    int *d_bins;
+    float2 *d_tw;
+};
+
+extern "C" int pdm_tf_destroy(pdm_tf *tf)
+{
+    if (!tf) return PDM_OK;
+    cudaFree(tf->d_bins); cudaFree(tf->d_tw);
+    delete tf;
+    return PDM_OK;
+}
+
+extern "C" int pdm_tf_create(pdm_tf **out, int nt, int nx, int nw, const int *bins)
+{
+    if (!out) return PDM_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!bins || nt <= 0 || nx <= 0 || nw <= 0) return PDM_ERR_INVALID_ARG;
+    for (int j = 0; j < nw; ++j)
+        if (bins[j] < 0 || bins[j] > nt / 2) return PDM_ERR_INVALID_ARG;
+    if (nt > PDM_TF_MAX_NT || (double)nw * (double)nx > 2.0e9 || (double)nt * (double)nx > 8.0e9)
+        return PDM_ERR_UNSUPPORTED;
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) {
+        cudaGetLastError();
+        return PDM_ERR_UNSUPPORTED;                        // no usable CUDA device: no fallback
+    }
+    if (prop.major != 10) return PDM_ERR_UNSUPPORTED;
+    pdm_tf *tf = new (std::nothrow) pdm_tf();
+    if (!tf) return PDM_ERR_NOMEM;
+    memset(tf, 0, sizeof(*tf));
+    tf->nt = nt; tf->nx = nx; tf->nw = nw; tf->device = dev;
+    tf->smem_bytes = ((nt + 1) & ~1) * (int)sizeof(float2) + 2 * PDM_TF_NC * PDM_TF_XB * (int)sizeof(float) +
+                     2 * (PDM_TF_THREADS / 32) * PDM_TF_JT * PDM_TF_NC * (int)sizeof(float2);
+    std::vector<float2> tw(nt);
+    const double two_pi = 6.283185307179586476925286766559;
+    for (int m = 0; m < nt; ++m) {                         // exact argument, one rounding to FP32
+        const double a = two_pi * (double)m / (double)nt;
+        tw[m] = make_float2((float)cos(a), (float)(-sin(a)));
+    }
+    bool ok = cudaMalloc((void **)&tf->d_bins, (size_t)nw * sizeof(int)) == cudaSuccess &&
+              cudaMalloc((void **)&tf->d_tw, (size_t)nt * sizeof(float2)) == cudaSuccess &&
+              cudaMemcpy(tf->d_bins, bins, (size_t)nw * sizeof(int), cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaMemcpy(tf->d_tw, tw.data(), (size_t)nt * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess &&
+              cudaFuncSetAttribute((const void *)pdm_tf_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   tf->smem_bytes) == cudaSuccess &&
+              cudaFuncSetAttribute((const void *)pdm_tf_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                   tf->smem_bytes) == cudaSuccess;
+    if (!ok) { cudaGetLastError(); pdm_tf_destroy(tf); return PDM_ERR_CUDA; }
+    // warps per CTA (4 bins each): all tiles take the same time, so pick the CTA height that wastes
+    // the least of the last wave
+    double best = -1.0;
+    const int xtiles = (nx + PDM_TF_XB - 1) / PDM_TF_XB;
+    for (int w = 8; w >= 4; --w) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)pdm_tf_kernel<4>, 32 * w,
+                                                          (size_t)tf->smem_bytes) != cudaSuccess || per_sm < 1)
+            continue;
+        const long long tiles = (long long)xtiles * ((nw + 4 * w - 1) / (4 * w));
+        const long long slots = (long long)prop.multiProcessorCount * per_sm;
+        const double eff = (double)nw * xtiles / (4.0 * w) / (double)(slots * ((tiles + slots - 1) / slots))
+                           * (w * per_sm >= 12 ? 1.0 : 0.8);      // fewer than 12 warps per SM: latency-bound
+        if (eff > best) { best = eff; tf->warps = w; }
+    }
+    if (best < 0.0) { cudaGetLastError(); pdm_tf_destroy(tf); return PDM_ERR_UNSUPPORTED; }
+    *out = tf;
+    return PDM_OK;
+}
+
+extern "C" int pdm_tf_forward(pdm_tf *tf, const float *section_dev, pdm_c64 *P0_dev, void *cuda_stream)
+{
+    if (!tf || !section_dev || !P0_dev) return PDM_ERR_INVALID_ARG;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != tf->device) { cudaGetLastError(); return PDM_ERR_CUDA; }
+    pdm_tf_params a;
+    a.section = section_dev; a.out = reinterpret_cast<float2 *>(P0_dev);
+    a.bins = tf->d_bins; a.tw = tf->d_tw; a.nt = tf->nt; a.nx = tf->nx; a.nw = tf->nw;
+    const int jb = tf->warps * PDM_TF_JT;
+    dim3 grid((tf->nx + PDM_TF_XB - 1) / PDM_TF_XB, (tf->nw + jb - 1) / jb);
+    if (tf->nx % 4 == 0 && ((uintptr_t)section_dev & 15u) == 0)
+        pdm_tf_kernel<4><<<grid, 32 * tf->warps, tf->smem_bytes, (cudaStream_t)cuda_stream>>>(a);
+    else
+        pdm_tf_kernel<1><<<grid, 32 * tf->warps, tf->smem_bytes, (cudaStream_t)cuda_stream>>>(a);
+    if (cudaGetLastError() != cudaSuccess) return PDM_ERR_CUDA;
+    return PDM_OK;
+}

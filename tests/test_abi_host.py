@@ -118,3 +118,16 @@ def test_product_package_never_imports_the_oracle():
         if f.endswith((".py", ".c")):
             text = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1912_05529_b200" not in text and "libpdm.so" not in text, f
+
+
+def test_tf_create_rejects_bad_arguments_before_touching_the_device(lib):
+    import numpy as np
+    import paper_1912_05529_b200 as pdm
+    ok = np.array([1, 2, 3], dtype=np.int32)
+    assert pdm.pdm_tf_create(0, 8, 3, ok)[0] == pdm.PDM_ERR_INVALID_ARG
+    assert pdm.pdm_tf_create(16, 0, 3, ok)[0] == pdm.PDM_ERR_INVALID_ARG
+    assert pdm.pdm_tf_create(16, 8, 0, ok[:0])[0] == pdm.PDM_ERR_INVALID_ARG
+    assert pdm.pdm_tf_create(16, 8, 3, np.array([1, 9, 3], dtype=np.int32))[0] == pdm.PDM_ERR_INVALID_ARG
+    assert pdm.pdm_tf_create(16, 8, 3, np.array([1, -1, 3], dtype=np.int32))[0] == pdm.PDM_ERR_INVALID_ARG
+    assert pdm.pdm_tf_create(1 << 14, 8, 3, ok)[0] == pdm.PDM_ERR_UNSUPPORTED      # nt > PDM_TF_MAX_NT
+    assert pdm.pdm_tf_destroy(None) == pdm.PDM_OK
