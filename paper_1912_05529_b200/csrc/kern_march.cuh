@@ -58,7 +58,7 @@ __device__ __forceinline__ float2 f4hi(float4 v) { return make_float2(v.z, v.w);
 // packed operand and the folded sample as the scalar one: the tap pair is then the same register
 // pair for up to 2R consecutive FFMA2 (register-reuse cache), which keeps the register-file reads
 // per instruction at <= 2 per bank; the scalar-tap form measured 0.80 of the pipe at best.
-template <int L, int R, bool UNIFORM>
+template <int L, int R, bool UNIFORM, bool DEDUP>
 __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
                                               const float4 *__restrict__ tbase,
                                               const int (&toff)[R], float2 (&out)[R])
@@ -71,8 +71,17 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
         wl[2 * i] = f4lo(v); wl[2 * i + 1] = f4hi(v);
         wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
     }
+    // DEDUP (plans whose model gives nearly every sample its own row, i.e. the tap gather is the
+    // bound): consecutive outputs of a thread still repeat a row often enough (smooth models) that
+    // fetching a row only where it differs from the previous output's (predicated loads) pays.
+    bool same[R];
 #pragma unroll
-    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r]];
+    for (int r = 0; r < R; ++r) same[r] = DEDUP && !UNIFORM && r > 0 && toff[r] == toff[r - 1];
+#pragma unroll
+    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) {
+        if (DEDUP && r > 0) tw[r] = tw[r - 1];
+        if (!same[r]) tw[r] = tbase[toff[r]];
+    }
 #pragma unroll
     for (int r = 0; r < R; ++r) {                       // centre tap W_0
         const float4 t = tw[UNIFORM ? 0 : r];
@@ -91,7 +100,10 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
             wl[pdm_mod(-k, R)] = f4lo(lv);
             wr[pdm_mod(k - 1, R)] = f4hi(rv);
 #pragma unroll
-            for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r] + k / 2];
+            for (int r = 0; r < (UNIFORM ? 1 : R); ++r) {
+                if (DEDUP && r > 0) tw[r] = tw[r - 1];
+                if (!same[r]) tw[r] = tbase[toff[r] + k / 2];
+            }
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -106,7 +118,7 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
     for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
 }
 
-template <int L, int R, bool TAPS_SMEM>
+template <int L, int R, bool TAPS_SMEM, bool DEDUP>
 __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(const pdm_march_params p)
 {
     static_assert(R % 2 == 0 && R >= 2, "R must be even");
@@ -254,8 +266,8 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                     }
                     const float2 *base = cur + (HG + g) * GS;
                     float2 out[R];
-                    if (uni) pdm_fir_group<L, R, true>(base, tbase, toff, out);
-                    else     pdm_fir_group<L, R, false>(base, tbase, toff, out);
+                    if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
+                    else     pdm_fir_group<L, R, false, DEDUP>(base, tbase, toff, out);
                     if (active) {
                         const int x0 = g * R;
                         float2 *dst = nxt + (HG + g) * GS;

@@ -115,8 +115,8 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         for (int r = 0; r < R; ++r) toff[r] = j[r] * p.half16;
         const float2 *base = ibuf + b * IN_SLOTS + (HG + lane) * GS;
         float2 out[R];
-        if (__all_sync(0xffffffffu, uni)) pdm_fir_group<L, R, true>(base, p.half, toff, out);
-        else                              pdm_fir_group<L, R, false>(base, p.half, toff, out);
+        if (__all_sync(0xffffffffu, uni)) pdm_fir_group<L, R, true, false>(base, p.half, toff, out);
+        else                              pdm_fir_group<L, R, false, false>(base, p.half, toff, out);
 
         float2 *od = obuf + lane * GS;
 #pragma unroll
