@@ -285,7 +285,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": {"workload": workload_name(args.config, cfg, world),
-                          "path": {1: "smem-marching", 2: "x-tiled", 3: "naive"}.get(info["path"]),
+                          "path": {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster"}.get(info["path"]),
                           "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                           "smem_bytes": info["smem_bytes"],
                           "l2": "256 MiB buffer written between timed steps (L2 flush); per-step "
@@ -359,7 +359,7 @@ def run_sweep(args):
                 sps = info["samples"] / t
                 tiled = info["path"] == pdm.PDM_PATH_TILED
                 out = {"workload": f"configs[4] nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} velocity={args.sweep_model}",
-                       "path": {1: "smem-marching", 2: "x-tiled", 3: "naive"}.get(info["path"]),
+                       "path": {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster"}.get(info["path"]),
                        "taps_mode": info["taps_mode"], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                        "launches": info["launches_per_migrate"], "steps": steps, "ms": t * 1e3,
                        "samples_per_s": sps,

@@ -9,7 +9,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpdm.so")
 SOURCES = ["pdm_api.cu"]
-HEADERS = ["pdm_common.cuh", "kern_naive.cuh", "kern_peak.cuh", "kern_march.cuh", "kern_tiled.cuh", "kern_tf.cuh"]
+HEADERS = ["pdm_common.cuh", "kern_naive.cuh", "kern_peak.cuh", "kern_march.cuh", "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-shared", "-Xcompiler", "-fPIC"]
 

@@ -15,6 +15,7 @@
 #include "kern_peak.cuh"
 #include "kern_march.cuh"
 #include "kern_tiled.cuh"
+#include "kern_cluster.cuh"
 
 #define PDM_CUDA(plan, call)                                                        \
     do {                                                                            \
@@ -141,6 +142,7 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
 #define PDM_R 8
 typedef void (*march_fn)(const pdm_march_params);
 typedef void (*tiled_fn)(const pdm_tiled_params);
+typedef void (*cluster_fn)(const pdm_cluster_params);
 
 #define PDM_FOR_EACH_L(X) X(1) X(2) X(3) X(7) X(12) X(15) X(17) X(25)
 
@@ -149,6 +151,15 @@ static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false)
     switch (L) {
 #define X(LL) case LL: return taps_smem ? (dedup ? pdm_march_kernel<LL, PDM_R, true, true> : pdm_march_kernel<LL, PDM_R, true, false>) \
                                          : (dedup ? pdm_march_kernel<LL, PDM_R, false, true> : pdm_march_kernel<LL, PDM_R, false, false>);
+        PDM_FOR_EACH_L(X)
+#undef X
+    default: return nullptr;
+    }
+}
+static cluster_fn cluster_kernel_for(int L, bool taps_smem)
+{
+    switch (L) {
+#define X(LL) case LL: return taps_smem ? pdm_cluster_kernel<LL, PDM_R, true> : pdm_cluster_kernel<LL, PDM_R, false>;
         PDM_FOR_EACH_L(X)
 #undef X
     default: return nullptr;
@@ -302,10 +313,38 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     const bool slice_fits = lines_fit && line_bytes + slice_bytes <= (size_t)p->smem_optin &&
                             p->max_rows <= 65535;
 
-    if (want == PDM_PATH_CLUSTER) return PDM_ERR_UNSUPPORTED;       // not built in this round
+    // cluster form: C = 2, 4 or 8 CTAs per line (bits PDM_CTAS_SHIFT force it).  Among the sizes
+    // whose per-CTA ping-pong segment fits shared memory, the largest that still leaves every CTA
+    // >= 256 groups and keeps nw*C within one wave of SMs, else the smallest that fits.
+    int cl_C = 0, cl_passes = 0, cl_nwarps = 0, cl_gper = 0;
+    size_t cl_seg_bytes = 0;
+    if (have_L) {
+        const unsigned csel = (want == PDM_PATH_CLUSTER) ? ((p->flags >> PDM_CTAS_SHIFT) & 0xFu) : 0u;
+        for (int c = 2; c <= 8; c *= 2) {
+            if (csel && (int)csel != c) continue;
+            const int gneed = (ngroups + c - 1) / c;
+            const int ps = (gneed + PDM_MARCH_MAX_THREADS - 1) / PDM_MARCH_MAX_THREADS;
+            const int nwp = (gneed + 32 * ps - 1) / (32 * ps);
+            const int gp = 32 * ps * nwp;
+            const size_t bytes = (size_t)2 * (2 * HG + gp) * (R + 2) * sizeof(float2) + (size_t)map_len * 2;
+            if (bytes > (size_t)p->smem_optin) continue;
+            const bool wanted = (long long)nw * c <= p->sm_count && gneed >= 256;
+            if (cl_C && !wanted) break;                    // keep the smaller size found before
+            cl_C = c; cl_passes = ps; cl_nwarps = nwp; cl_gper = gp; cl_seg_bytes = bytes;
+            if (!wanted) break;                            // smallest that fits
+        }
+    }
+    const bool cl_slice_ok = cl_C && cl_seg_bytes + slice_bytes <= (size_t)p->smem_optin && p->max_rows <= 65535;
+    // AUTO takes the cluster form when there are too few lines to give every SM a CTA (measured
+    // 1.3-1.8x on configs[4] nw = 64 points with nx >= 4096) and the tap rows can still be staged
+    const bool auto_cluster = cl_slice_ok && 2 * nw <= p->sm_count && ngroups >= 512 &&
+                              (long long)nw * cl_C <= 2LL * p->sm_count;
+    if (want == PDM_PATH_CLUSTER && !cl_C) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;  // (tiled_kernel_for has the same L list)
-    if (want == PDM_PATH_AUTO) p->path = lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE);
+    if (want == PDM_PATH_AUTO)
+        p->path = auto_cluster ? PDM_PATH_CLUSTER
+                               : (lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE));
     else p->path = (int)want;
 
     int rc;
@@ -356,6 +395,41 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
             if ((rc = dev_alloc(p, &p->d_flags, (size_t)std::max(1, p->nslots))) != PDM_OK) return rc;
             PDM_CUDA(p, cudaMemset(p->d_flags, 0, (size_t)std::max(1, p->nslots) * sizeof(int)));
         }
+        if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->n_partial * nz * (ngroups * R))) != PDM_OK) return rc;
+    } else if (p->path == PDM_PATH_CLUSTER) {
+        const int C = cl_C, passes = cl_passes, nwarps = cl_nwarps, gper = cl_gper;
+        const size_t seg_bytes = cl_seg_bytes;
+        const bool slice_ok = cl_slice_ok;
+        if (want_taps == PDM_TAPS_SLICE || want_taps == PDM_TAPS_COMPACT) {
+            if (!slice_ok) return PDM_ERR_UNSUPPORTED;
+            p->taps_in_smem = 1;
+        } else if (want_taps == PDM_TAPS_GLOBAL) p->taps_in_smem = 0;
+        else p->taps_in_smem = slice_ok ? 1 : 0;
+        p->taps_mode = p->taps_in_smem ? (p->contiguous_rows ? 2 : 3) : 1;
+        p->threads = 32 * nwarps;
+        p->cluster_size = C; p->cluster_gper = gper; p->cluster_passes = passes;
+        p->smem_bytes = (int)(seg_bytes + (p->taps_in_smem ? slice_bytes : 0));
+        cluster_fn fn = cluster_kernel_for(L, p->taps_in_smem != 0);
+        PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         p->smem_bytes));
+        int max_clusters = 0;
+        {
+            cudaLaunchConfig_t cfg = {};
+            cudaLaunchAttribute at[1];
+            at[0].id = cudaLaunchAttributeClusterDimension;
+            at[0].val.clusterDim.x = C; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+            cfg.gridDim = dim3(C * p->sm_count); cfg.blockDim = dim3(p->threads);
+            cfg.dynamicSmemBytes = (size_t)p->smem_bytes; cfg.attrs = at; cfg.numAttrs = 1;
+            PDM_CUDA(p, cudaOccupancyMaxActiveClusters(&max_clusters, (const void *)fn, &cfg));
+        }
+        if (max_clusters < 1) return PDM_ERR_UNSUPPORTED;
+        p->ctas_per_sm = 1;
+        p->n_partial = std::min(nw, max_clusters);
+        p->grid = p->n_partial * C;
+        p->launches = 2;
         if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
@@ -436,6 +510,30 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
             fn<<<p->grid, p->threads, p->smem_bytes, st>>>(a);
         }
         PDM_CUDA(p, cudaGetLastError());
+        if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[1], st));
+        dim3 rg((nx + 255) / 256, nz);
+        pdm_reduce_partials<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->n_partial, nz, nx, a.pstride);
+        PDM_CUDA(p, cudaGetLastError());
+    } else if (p->path == PDM_PATH_CLUSTER) {
+        pdm_cluster_params a;
+        a.P0 = P0; a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega;
+        a.half = p->d_half; a.rowoff = p->d_rowoff; a.rows = p->d_rows;
+        a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
+        a.ngroups = (nx + R - 1) / R;
+        a.qstride = p->qstride; a.pstride = a.ngroups * R; a.half16 = p->half16;
+        a.passes = p->cluster_passes; a.gper = p->cluster_gper;
+        a.slots = (2 * halo_groups(L, R) + a.gper) * (R + 2);
+        a.map_len = round_up(p->ntab, 8);
+        a.nclusters = p->n_partial;
+        cluster_fn fn = cluster_kernel_for(L, p->taps_in_smem != 0);
+        cudaLaunchConfig_t cfg = {};
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = p->cluster_size; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.gridDim = dim3(p->grid); cfg.blockDim = dim3(p->threads);
+        cfg.dynamicSmemBytes = (size_t)p->smem_bytes; cfg.stream = st; cfg.attrs = at; cfg.numAttrs = 1;
+        if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
+        PDM_CUDA(p, cudaLaunchKernelEx(&cfg, fn, a));
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[1], st));
         dim3 rg((nx + 255) / 256, nz);
         pdm_reduce_partials<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->n_partial, nz, nx, a.pstride);

@@ -55,14 +55,15 @@ def assert_parity(pdm, cfg, flags=0, ref=None, expect_path=None):
     return rel, mx
 
 
-PATHS = ["naive", "smem_global", "smem_staged", "tiled"]
+PATHS = ["naive", "smem_global", "smem_staged", "tiled", "cluster"]
 
 
 def path_flags(pdm, name):
     return {"naive": pdm.PDM_PATH_NAIVE,
             "smem_global": pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_GLOBAL,
             "smem_staged": pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_SLICE,
-            "tiled": pdm.PDM_PATH_TILED}[name]
+            "tiled": pdm.PDM_PATH_TILED,
+            "cluster": pdm.PDM_PATH_CLUSTER}[name]
 
 
 # ---------------------------------------------------------------- every kernel form, small inputs
@@ -165,6 +166,31 @@ def test_tiled_path_with_unaligned_plane_pointer(pdm):
     assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
 
 
+@pytest.mark.parametrize("nx,nz,nw,ntaps,model,csize", [
+    (1000, 24, 5, 25, "white", 4),       # 125 groups over 4 CTAs of one warp: ragged last CTA
+    (129, 50, 3, 35, "const", 8),        # 17 groups over 8 CTAs: most CTAs of a cluster idle
+    (9000, 20, 300, 25, "layers", 4),    # more lines than clusters: partial-image accumulation
+    (20000, 10, 3, 15, "field", 0),      # a line too long for one CTA: auto cluster size
+    (4100, 12, 4, 51, "field", 2),       # halo of 4 groups pushed through DSMEM, 2 passes per CTA
+])
+def test_cluster_path_matches_oracle(pdm, nx, nz, nw, ntaps, model, csize):
+    """Line split over a thread-block cluster: halos pushed into the neighbour CTA's shared memory,
+    step counters published with release.cluster stores; parity and bit-identical repeats."""
+    import torch
+    cfg = pdm_inputs.random_problem(13, nx, nz, nw, ntaps, model=model)
+    flags = pdm.PDM_PATH_CLUSTER | (csize << pdm.PDM_CTAS_SHIFT)
+    ref = oracle.migrate(cfg)
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        assert plan.info["path"] == pdm.PDM_PATH_CLUSTER
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(p0).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    rel, mx = errors(a.cpu().numpy(), ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+
+
 # ---------------------------------------------------------------- BASELINE.json configs
 def test_config0_all_paths(pdm, config0):
     ref = oracle.migrate(config0)
@@ -212,8 +238,12 @@ def test_config3_full_size_sampled_frequencies(pdm):
 def test_config4_points_sampled_frequencies(pdm, nx, nw, ntaps):
     cfg = pdm_inputs.sweep_point(nx, nw, ntaps)
     lines = sorted({0, nw // 3, nw - 1})
-    _subset_parity(pdm, cfg, lines, 0,
-                   expect_path=pdm.PDM_PATH_TILED if nx >= 16384 else pdm.PDM_PATH_SMEM)
+    # nx >= 16384 cannot be a single-CTA line: x-tiled, or (few lines, rows stageable) the cluster form
+    _subset_parity(pdm, cfg, lines, 0, expect_path=None if nx >= 16384 else pdm.PDM_PATH_SMEM)
+    if nx >= 16384:
+        with pdm.Plan.from_config(cfg, 0) as plan:
+            assert plan.info["path"] in (pdm.PDM_PATH_TILED, pdm.PDM_PATH_CLUSTER)
+        _subset_parity(pdm, cfg, lines, pdm.PDM_PATH_TILED, expect_path=pdm.PDM_PATH_TILED)
 
 
 # ---------------------------------------------------------------- properties of the GPU path itself
@@ -282,8 +312,8 @@ def test_error_codes_on_device(pdm):
     args = (c["nx"], c["nz"], c["nw"], c["dx"], c["dz"], c["omega"], c["velocity"], c["table"])
     rc, h = pdm.pdm_create(*args, c["du"] * 0.5)                     # u exceeds the table
     assert rc == pdm.PDM_ERR_TABLE_RANGE and h is None
-    rc, h = pdm.pdm_create(*args, c["du"], pdm.PDM_PATH_CLUSTER)
-    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
+    rc, h = pdm.pdm_create(*args, c["du"], pdm.PDM_PATH_CLUSTER | (3 << pdm.PDM_CTAS_SHIFT))
+    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None              # cluster sizes are 2, 4, 8
     big = pdm_inputs.random_problem(1, 40000, 2, 1, 15, model="const")
     rc, h = pdm.pdm_create(big["nx"], big["nz"], big["nw"], big["dx"], big["dz"], big["omega"],
                            big["velocity"], big["table"], big["du"], pdm.PDM_PATH_SMEM)
