@@ -206,7 +206,12 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(c
                             *reinterpret_cast<const float4 *>(nxt + (p.gper + gg) * GS + 2 * c);
                     }
                 }
-                asm volatile("fence.acq_rel.cluster;" ::: "memory");
+                // only the two edge warps wrote into another CTA: the cluster-scope fence (which also
+                // invalidates L1) is theirs alone, interior warps order their step with a CTA fence
+                if ((warp == 0 && left_active) || (warp == nwarps - 1 && right_active))
+                    asm volatile("fence.acq_rel.cluster;" ::: "memory");
+                else
+                    __threadfence_block();
                 __syncwarp();
                 if (lane == 0) {                           // A4: publish this warp's step z
                     const int done = z + 1;
