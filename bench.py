@@ -41,8 +41,8 @@ UNIT = "samples/s"
 FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
 # committed `ncu --set full` capture of this command (profiles/r01_march_config3.md, section 2):
-# 27.23 GB + 29.55 GB on configs[3] (the per-CTA partial-image read-modify-write).
-NCU_DRAM_BYTES_PER_LAUNCH = {3: 27.230737e9 + 29.551742e9}
+# 27.09 GB + 29.55 GB on configs[3] (the per-CTA partial-image read-modify-write).
+NCU_DRAM_BYTES_PER_LAUNCH = {3: 27.094569e9 + 29.553966e9}
 
 
 def load_workload(k: int, rank: int, world: int) -> dict:
