@@ -13,9 +13,8 @@
 #include "pdm_common.cuh"
 #include "kern_naive.cuh"
 #include "kern_peak.cuh"
-#include "kern_march.cuh"
-#include "kern_tiled.cuh"
-#include "kern_cluster.cuh"
+#include "kern_reduce.cuh"
+#include "pdm_dispatch.cuh"
 
 #define PDM_CUDA(plan, call)                                                        \
     do {                                                                            \
@@ -139,41 +138,15 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
 // ------------------------------------------------------------------------------------------------
 // kernel dispatch: filter half-lengths with a fully unrolled, register-tiled instantiation
 // ------------------------------------------------------------------------------------------------
-#define PDM_R 8
-typedef void (*march_fn)(const pdm_march_params);
-typedef void (*tiled_fn)(const pdm_tiled_params);
-typedef void (*cluster_fn)(const pdm_cluster_params);
-
-#define PDM_FOR_EACH_L(X) X(1) X(2) X(3) X(7) X(12) X(15) X(17) X(25)
-
 static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false)
 {
-    switch (L) {
-#define X(LL) case LL: return taps_smem ? (dedup ? pdm_march_kernel<LL, PDM_R, true, true> : pdm_march_kernel<LL, PDM_R, true, false>) \
-                                         : (dedup ? pdm_march_kernel<LL, PDM_R, false, true> : pdm_march_kernel<LL, PDM_R, false, false>);
-        PDM_FOR_EACH_L(X)
-#undef X
-    default: return nullptr;
-    }
+    march_fn f = pdm_march_kernel_part0(L, taps_smem, dedup);
+    if (!f) f = pdm_march_kernel_part1(L, taps_smem, dedup);
+    if (!f) f = pdm_march_kernel_part2(L, taps_smem, dedup);
+    return f;
 }
-static cluster_fn cluster_kernel_for(int L, bool taps_smem)
-{
-    switch (L) {
-#define X(LL) case LL: return taps_smem ? pdm_cluster_kernel<LL, PDM_R, true> : pdm_cluster_kernel<LL, PDM_R, false>;
-        PDM_FOR_EACH_L(X)
-#undef X
-    default: return nullptr;
-    }
-}
-static tiled_fn tiled_kernel_for(int L, bool wide)
-{
-    switch (L) {
-#define X(LL) case LL: return wide ? pdm_tiled_step<LL, PDM_R, 2> : pdm_tiled_step<LL, PDM_R, 1>;
-        PDM_FOR_EACH_L(X)
-#undef X
-    default: return nullptr;
-    }
-}
+static cluster_fn cluster_kernel_for(int L, bool taps_smem) { return pdm_cluster_kernel_for(L, taps_smem); }
+static tiled_fn tiled_kernel_for(int L, bool wide) { return pdm_tiled_kernel_for(L, wide); }
 // Work list of the marching kernel.  Unbalanced: CTA c owns whole lines c, c+grid, ...  Balanced
 // (nw >= grid): the nw*nz depth steps, laid end to end line after line, are cut into `grid` equal
 // ranges; a range is [tail of a line][whole lines][head of a line].  The CTA runs its head FIRST
