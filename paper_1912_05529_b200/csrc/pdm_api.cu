@@ -146,7 +146,9 @@ static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false)
     return f;
 }
 static cluster_fn cluster_kernel_for(int L, bool taps_smem) { return pdm_cluster_kernel_for(L, taps_smem); }
-static tiled_fn tiled_kernel_for(int L, bool wide) { return pdm_tiled_kernel_for(L, wide); }
+// output tile aliased onto the consumed input tile: only where it pays (long per-sample rows)
+static bool tiled_alias(const pdm_plan *p) { return p->contiguous_rows != 0 && p->L == 25; }
+static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide) { return pdm_tiled_kernel_for(p->L, wide, tiled_alias(p)); }
 // Work list of the marching kernel.  Unbalanced: CTA c owns whole lines c, c+grid, ...  Balanced
 // (nw >= grid): the nw*nz depth steps, laid end to end line after line, are cut into `grid` equal
 // ranges; a range is [tail of a line][whole lines][head of a line].  The CTA runs its head FIRST
@@ -412,11 +414,11 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->threads = PDM_TILED_THREADS;
         p->tile_x = PDM_TILED_THREADS * R;
         const int xtiles = (nx + p->tile_x - 1) / p->tile_x;
-        // per warp: double-buffered input sub-tile (+ halos) and one output sub-tile
-        p->smem_bytes = (PDM_TILED_THREADS / 32) * (2 * (32 + 2 * HG) + 32) * (R + 2) * (int)sizeof(float2);
+        // per warp: double-buffered input sub-tile (+ halos) and an output sub-tile (unless aliased)
+        p->smem_bytes = (PDM_TILED_THREADS / 32) * (2 * (32 + 2 * HG) + (tiled_alias(p) ? 0 : 32)) * (R + 2) * (int)sizeof(float2);
         int per_sm = 0;
         for (int wide = 0; wide < 2; ++wide) {
-            tiled_fn fn = tiled_kernel_for(L, wide != 0);
+            tiled_fn fn = tiled_kernel_for(p, wide != 0);
             PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              p->smem_bytes));
             PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn,
@@ -519,7 +521,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.w_per_group = (nw + p->wgroups - 1) / p->wgroups;
         // 16-byte async copies need every plane row 16-byte aligned: nx even and an aligned P0
         const bool wide = (nx % 2 == 0) && (((uintptr_t)P0_dev & 15u) == 0);
-        tiled_fn fn = tiled_kernel_for(L, wide);
+        tiled_fn fn = tiled_kernel_for(p, wide);
         dim3 grid((nx + p->tile_x - 1) / p->tile_x, p->wgroups);
         const float2 *src = P0;
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));

@@ -21,4 +21,4 @@ march_fn pdm_march_kernel_part0(int L, bool taps_smem, bool dedup);
 march_fn pdm_march_kernel_part1(int L, bool taps_smem, bool dedup);
 march_fn pdm_march_kernel_part2(int L, bool taps_smem, bool dedup);
 cluster_fn pdm_cluster_kernel_for(int L, bool taps_smem);
-tiled_fn pdm_tiled_kernel_for(int L, bool wide);
+tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias);

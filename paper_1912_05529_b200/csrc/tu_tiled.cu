@@ -1,10 +1,11 @@
 // tu_tiled.cu -- instantiations of pdm_tiled_step (see pdm_dispatch.cuh).
 #include "pdm_dispatch.cuh"
 
-tiled_fn pdm_tiled_kernel_for(int L, bool wide)
+tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias)
 {
+    if (alias && L == 25) return wide ? pdm_tiled_step<25, PDM_R, 2, true> : pdm_tiled_step<25, PDM_R, 1, true>;
     switch (L) {
-#define X(LL) case LL: return wide ? pdm_tiled_step<LL, PDM_R, 2> : pdm_tiled_step<LL, PDM_R, 1>;
+#define X(LL) case LL: return wide ? pdm_tiled_step<LL, PDM_R, 2, false> : pdm_tiled_step<LL, PDM_R, 1, false>;
         PDM_FOR_EACH_L(X)
 #undef X
     default: return nullptr;
