@@ -257,6 +257,35 @@ def test_delta_table_is_identity_on_gpu(pdm):
             np.testing.assert_allclose(img[z], want, rtol=0, atol=1e-5)
 
 
+@pytest.mark.parametrize("path", PATHS)
+def test_gpu_path_properties_superposition_mirror_additivity(pdm, path):
+    """Properties that hold for the method at any size, checked on the GPU path itself (no oracle):
+    real-linear superposition, x-mirror symmetry (symmetric taps + zero edges), and additivity over
+    a split of the frequency list."""
+    flags = path_flags(pdm, path)
+    cfg = pdm_inputs.random_problem(37, 777, 14, 6, 25, model="field")
+    rng = np.random.default_rng(5)
+    A = cfg["P0"]
+    B = (rng.standard_normal(A.shape) + 1j * rng.standard_normal(A.shape)).astype(np.complex64)
+    img_a = gpu_migrate(pdm, cfg, flags).astype(np.float64)
+    img_b = gpu_migrate(pdm, cfg, flags, P0=B).astype(np.float64)
+    img_c = gpu_migrate(pdm, cfg, flags, P0=(2.0 * A - 0.5 * B).astype(np.complex64)).astype(np.float64)
+    scale = np.abs(img_a).max() + np.abs(img_b).max()
+    assert np.abs(img_c - (2.0 * img_a - 0.5 * img_b)).max() <= 2e-5 * scale
+    # mirror: reverse x in the data and in the velocity -> the image is reversed
+    mir = dict(cfg, velocity=np.ascontiguousarray(cfg["velocity"][:, ::-1]))
+    img_m = gpu_migrate(pdm, mir, flags, P0=np.ascontiguousarray(A[:, ::-1])).astype(np.float64)
+    assert np.abs(img_m[:, ::-1] - img_a).max() <= 2e-5 * np.abs(img_a).max()
+    # frequency additivity: image(all) = image(first half) + image(second half)
+    h = cfg["nw"] // 2
+    parts = []
+    for sl in (slice(0, h), slice(h, None)):
+        sub = dict(cfg, omega=np.ascontiguousarray(cfg["omega"][sl]), nw=len(cfg["omega"][sl]),
+                   P0=np.ascontiguousarray(A[sl]))
+        parts.append(gpu_migrate(pdm, sub, flags).astype(np.float64))
+    assert np.abs(parts[0] + parts[1] - img_a).max() <= 2e-5 * np.abs(img_a).max()
+
+
 def test_repeated_migrate_is_bit_identical_and_plans_are_independent(pdm):
     import torch
     a = pdm_inputs.random_problem(21, 700, 20, 300, 15, model="field")
