@@ -286,6 +286,36 @@ def test_gpu_path_properties_superposition_mirror_additivity(pdm, path):
     assert np.abs(parts[0] + parts[1] - img_a).max() <= 2e-5 * np.abs(img_a).max()
 
 
+@pytest.mark.parametrize("name,nx,nz,nw,ntaps,model,path", [
+    ("smem balanced", 700, 20, 300, 15, "field", "auto"),
+    ("smem whole lines", 333, 10, 5, 25, "layers", "smem_staged"),
+    ("tiled", 2600, 8, 6, 25, "field", "tiled"),
+    ("cluster", 5000, 8, 6, 25, "layers", "cluster"),
+])
+def test_migrate_is_cuda_graph_capturable(pdm, name, nx, nz, nw, ntaps, model, path):
+    """pdm_migrate only enqueues work (no allocation, no host sync, no copies): capture it in a CUDA
+    graph -- cooperative and cluster launches included -- and replay it."""
+    import torch
+    cfg = pdm_inputs.random_problem(43, nx, nz, nw, ntaps, model=model)
+    flags = 0 if path == "auto" else path_flags(pdm, path)
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        img = torch.empty((nz, nx), dtype=torch.float32, device="cuda")
+        ref = plan.migrate(p0).clone()
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        with torch.cuda.stream(s):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                plan.migrate(p0, img, stream=s)
+        img.zero_()
+        torch.cuda.synchronize()
+        g.replay()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(img, ref), name
+
+
 def test_repeated_migrate_is_bit_identical_and_plans_are_independent(pdm):
     import torch
     a = pdm_inputs.random_problem(21, 700, 20, 300, 15, model="field")
