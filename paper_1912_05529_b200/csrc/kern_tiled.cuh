@@ -19,6 +19,9 @@
 #include "kern_march.cuh"
 
 #define PDM_TILED_THREADS 256
+#ifndef PDM_TILED_STAGES
+#define PDM_TILED_STAGES 2      // input sub-tiles per warp (cp.async ring): STAGES-1 in flight; 3 measured 4-8 % slower
+#endif
 
 struct pdm_tiled_params {
     const float2 *Pin;       // [nw][nx] plane at depth z
@@ -51,7 +54,8 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
     constexpr int T = PDM_TILED_THREADS;
     constexpr int IN_SLOTS = (32 + 2 * HG) * GS;                  // per warp and buffer
     // two input buffers + an output tile; with ALIAS the consumed input buffer holds the results
-    constexpr int WARP_SLOTS = 2 * IN_SLOTS + (ALIAS ? 0 : 32 * GS);
+    constexpr int NB = PDM_TILED_STAGES;
+    constexpr int WARP_SLOTS = NB * IN_SLOTS + (ALIAS ? 0 : 32 * GS);
     extern __shared__ __align__(16) unsigned char pdm_smem[];
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     float2 *ibuf = reinterpret_cast<float2 *>(pdm_smem) + warp * WARP_SLOTS;   // [2][IN_SLOTS]
@@ -75,7 +79,9 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    if (w_begin < w_end) issue_load(w_begin, 0);
+#pragma unroll
+    for (int i = 0; i < NB - 1; ++i)
+        if (w_begin + i < w_end) issue_load(w_begin + i, i);
 
     float qc[R];
     {
@@ -92,15 +98,16 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
     for (int r = 0; r < R; ++r) img[r] = 0.f;
 
     for (int iw = w_begin, it = 0; iw < w_end; ++iw, ++it) {
-        const int b = it & 1;
+        const int b = it % NB;
         const float w = p.omega[iw];
         // the warp is past the compute of iteration it-1 (__syncwarp before its copy-out), so the
-        // buffer it read, b^1, may be refilled now
-        if (iw + 1 < w_end) {
-            issue_load(iw + 1, b ^ 1);
-            asm volatile("cp.async.wait_group 1;" ::: "memory");
-        } else {
-            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        // buffer it read, (it-1) % NB, may be refilled now (with the tile NB-1 frequencies ahead)
+        if (iw + NB - 1 < w_end) issue_load(iw + NB - 1, (it + NB - 1) % NB);
+        {                                                  // groups committed after tile iw's
+            const int ahead = min(NB - 1, w_end - 1 - iw);
+            if (ahead >= 2)      asm volatile("cp.async.wait_group 2;" ::: "memory");
+            else if (ahead == 1) asm volatile("cp.async.wait_group 1;" ::: "memory");
+            else                 asm volatile("cp.async.wait_group 0;" ::: "memory");
         }
         __syncwarp();                                      // tile of iw complete; obuf of it-1 drained
 
@@ -122,7 +129,7 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         // output tile -- less shared memory leaves more L1 for the tap rows (+11..24 % at 51 taps on
         // random-field models, -7 % where rows are warp-uniform, hence a per-plan choice); every
         // lane must be done reading its windows before anyone overwrites them
-        float2 *obuf = ALIAS ? ibuf + b * IN_SLOTS + HG * GS : ibuf + 2 * IN_SLOTS;
+        float2 *obuf = ALIAS ? ibuf + b * IN_SLOTS + HG * GS : ibuf + NB * IN_SLOTS;
         if (ALIAS) __syncwarp();
         float2 *od = obuf + lane * GS;
 #pragma unroll

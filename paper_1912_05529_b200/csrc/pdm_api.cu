@@ -415,7 +415,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->tile_x = PDM_TILED_THREADS * R;
         const int xtiles = (nx + p->tile_x - 1) / p->tile_x;
         // per warp: double-buffered input sub-tile (+ halos) and an output sub-tile (unless aliased)
-        p->smem_bytes = (PDM_TILED_THREADS / 32) * (2 * (32 + 2 * HG) + (tiled_alias(p) ? 0 : 32)) * (R + 2) * (int)sizeof(float2);
+        p->smem_bytes = (PDM_TILED_THREADS / 32) * (PDM_TILED_STAGES * (32 + 2 * HG) + (tiled_alias(p) ? 0 : 32)) * (R + 2) * (int)sizeof(float2);
         int per_sm = 0;
         for (int wide = 0; wide < 2; ++wide) {
             tiled_fn fn = tiled_kernel_for(p, wide != 0);
