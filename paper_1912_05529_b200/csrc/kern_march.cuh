@@ -247,6 +247,11 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(con
                     if (++qp == npw) { qp = 0; ++qz; }   // A1 prefetch: q two groups ahead
                     if (qz < z1) load_q(qz, qp);         // else: tn/un of groups that are never run
                     float4 *prow = reinterpret_cast<float4 *>(my_partial + (size_t)z * p.pstride + (size_t)g * R);
+                    // short filters: a group is over before a DRAM load returns, and the partial image
+                    // is far larger than L2 -- pull the NEXT depth step's row into L2 a step ahead
+                    // (+5 % at 15 taps; long filters hide the latency anyway and lose 1.5 % to it)
+                    if (L <= 15 && z + 1 < min(wz, z1))
+                        asm volatile("prefetch.global.L2 [%0];" :: "l"(reinterpret_cast<const float *>(prow) + p.pstride));
                     float4 pold[R / 4];
                     if (accumulate) {                    // A5: old partial row, consumed at the end
 #pragma unroll
