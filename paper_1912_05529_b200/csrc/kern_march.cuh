@@ -118,8 +118,10 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
     for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
 }
 
+// R = 8: one CTA of up to 384 threads per SM.  R = 4 (short lines, few of them): up to 256 threads and
+// at least two CTAs per SM, so that small problems put more warps on an SM.
 template <int L, int R, bool TAPS_SMEM, bool DEDUP>
-__global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_march_kernel(const pdm_march_params p)
+__global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ? 1 : 2) pdm_march_kernel(const pdm_march_params p)
 {
     static_assert(R % 2 == 0 && R >= 2, "R must be even");
     constexpr int HG = pdm_halo_groups<L, R>();

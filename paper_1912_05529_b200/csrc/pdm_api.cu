@@ -138,11 +138,11 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
 // ------------------------------------------------------------------------------------------------
 // kernel dispatch: filter half-lengths with a fully unrolled, register-tiled instantiation
 // ------------------------------------------------------------------------------------------------
-static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false)
+static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false, int R = PDM_R)
 {
-    march_fn f = pdm_march_kernel_part0(L, taps_smem, dedup);
-    if (!f) f = pdm_march_kernel_part1(L, taps_smem, dedup);
-    if (!f) f = pdm_march_kernel_part2(L, taps_smem, dedup);
+    march_fn f = pdm_march_kernel_part0(L, taps_smem, dedup, R);
+    if (!f) f = pdm_march_kernel_part1(L, taps_smem, dedup, R);
+    if (!f) f = pdm_march_kernel_part2(L, taps_smem, dedup, R);
     return f;
 }
 static cluster_fn cluster_kernel_for(int L, bool taps_smem) { return pdm_cluster_kernel_for(L, taps_smem); }
@@ -199,11 +199,17 @@ static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 static int build_plan(pdm_plan *p, const float *omega, const float *velocity, const pdm_c64 *table)
 {
     const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, ntaps = p->ntaps, L = p->L;
-    const int R = PDM_R;
+    // outputs per thread: 8, or 4 for short lines with so few of them that 8 would leave the SMs
+    // with under 8 warps each (configs[0], [1]); only the single-CTA marching form has the R = 4 build
+    const unsigned want_path = p->flags & PDM_PATH_MASK;
+    const bool small = (want_path == PDM_PATH_AUTO || want_path == PDM_PATH_SMEM) && nx <= 1024 &&
+                       (long long)nw * ((nx + 255) / 256) <= 8LL * p->sm_count &&
+                       ((p->flags >> PDM_THREADS_SHIFT) & 0xFFu) == 0;   // a forced thread count means the R = 8 layout
+    const int R = small ? PDM_R_SMALL : PDM_R;
     p->R = R;
 
     // ---- q map (R3) and its extrema ---------------------------------------------------------
-    p->qstride = round_up(nx, PDM_TILED_THREADS * R);
+    p->qstride = round_up(nx, PDM_TILED_THREADS * PDM_R);
     std::vector<float> q((size_t)nz * p->qstride);
     float qmin = INFINITY, qmax = 0.f;
     for (int z = 0; z < nz; ++z) {
@@ -334,16 +340,17 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         else p->taps_in_smem = slice_fits ? 1 : 0;
         p->taps_mode = p->taps_in_smem ? (p->contiguous_rows ? 2 : 3) : 1;
 
-        int passes = (ngroups + PDM_MARCH_MAX_THREADS - 1) / PDM_MARCH_MAX_THREADS;
+        const int max_threads = (R >= 8) ? PDM_MARCH_MAX_THREADS : 256;
+        int passes = (ngroups + max_threads - 1) / max_threads;
         int threads = round_up((ngroups + passes - 1) / passes, 32);
         const unsigned tsel = (p->flags >> PDM_THREADS_SHIFT) & 0xFFu;
         if (tsel) {
-            threads = std::min((int)tsel * 32, PDM_MARCH_MAX_THREADS);
+            threads = std::min((int)tsel * 32, max_threads);
             passes = (ngroups + threads - 1) / threads;
         }
         p->threads = threads;
         p->smem_bytes = (int)(line_bytes + (p->taps_in_smem ? slice_bytes : 0));
-        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0, use_dedup(p));
+        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0, use_dedup(p), R);
         PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          p->smem_bytes));
         int per_sm = 0;
@@ -475,7 +482,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.passes = (a.ngroups + p->threads - 1) / p->threads;
         a.slots = (2 * halo_groups(L, R) + a.ngroups) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
-        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0, use_dedup(p));
+        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0, use_dedup(p), R);
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
         if (p->balanced) {                               // split lines: CTAs wait on one another
             void *args[] = { (void *)&a };

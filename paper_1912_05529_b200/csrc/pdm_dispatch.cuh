@@ -17,8 +17,10 @@ typedef void (*cluster_fn)(const pdm_cluster_params);
 #define PDM_L_PART2(X) X(25)
 #define PDM_FOR_EACH_L(X) PDM_L_PART0(X) PDM_L_PART1(X) PDM_L_PART2(X)
 
-march_fn pdm_march_kernel_part0(int L, bool taps_smem, bool dedup);
-march_fn pdm_march_kernel_part1(int L, bool taps_smem, bool dedup);
-march_fn pdm_march_kernel_part2(int L, bool taps_smem, bool dedup);
+// R = outputs per thread: PDM_R, or PDM_R_SMALL for problems with too few warps to fill the SMs
+#define PDM_R_SMALL 4
+march_fn pdm_march_kernel_part0(int L, bool taps_smem, bool dedup, int R);
+march_fn pdm_march_kernel_part1(int L, bool taps_smem, bool dedup, int R);
+march_fn pdm_march_kernel_part2(int L, bool taps_smem, bool dedup, int R);
 cluster_fn pdm_cluster_kernel_for(int L, bool taps_smem);
 tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias);

@@ -13,13 +13,19 @@
 #define PDM_PART_FN pdm_march_kernel_part2
 #endif
 
-march_fn PDM_PART_FN(int L, bool taps_smem, bool dedup)
+template <int RR>
+static march_fn pick(int L, bool taps_smem, bool dedup)
 {
     switch (L) {
-#define X(LL) case LL: return taps_smem ? (dedup ? pdm_march_kernel<LL, PDM_R, true, true> : pdm_march_kernel<LL, PDM_R, true, false>) \
-                                         : (dedup ? pdm_march_kernel<LL, PDM_R, false, true> : pdm_march_kernel<LL, PDM_R, false, false>);
+#define X(LL) case LL: return taps_smem ? (dedup ? pdm_march_kernel<LL, RR, true, true> : pdm_march_kernel<LL, RR, true, false>) \
+                                         : (dedup ? pdm_march_kernel<LL, RR, false, true> : pdm_march_kernel<LL, RR, false, false>);
         PDM_L_THIS(X)
 #undef X
     default: return nullptr;
     }
+}
+
+march_fn PDM_PART_FN(int L, bool taps_smem, bool dedup, int R)
+{
+    return R == PDM_R_SMALL ? pick<PDM_R_SMALL>(L, taps_smem, dedup) : pick<PDM_R>(L, taps_smem, dedup);
 }
