@@ -316,6 +316,30 @@ def test_migrate_is_cuda_graph_capturable(pdm, name, nx, nz, nw, ntaps, model, p
         assert torch.equal(img, ref), name
 
 
+@pytest.mark.parametrize("name,nx,nz,nw,ntaps,model,path,csize", [
+    ("march balanced", 3000, 40, 500, 25, "layers", "auto", 0),
+    ("march dedup", 2048, 30, 320, 15, "field", "auto", 0),
+    ("march R=4", 512, 60, 100, 31, "layers", "auto", 0),
+    ("cluster of 4", 9000, 30, 40, 25, "layers", "cluster", 4),
+    ("cluster of 8", 20000, 20, 12, 15, "field", "cluster", 8),
+])
+def test_flag_synchronised_kernels_repeat_bit_identically(pdm, name, nx, nz, nw, ntaps, model, path, csize):
+    """The depth steps are ordered by progress flags (between warps, between CTAs of a cluster and,
+    with depth-split balancing, between CTAs through HBM), not by barriers: a missing fence would
+    show up as run-to-run differences.  60 repeats of full-machine grids must be bit-identical."""
+    import torch
+    cfg = pdm_inputs.random_problem(61, nx, nz, nw, ntaps, model=model)
+    flags = 0 if path == "auto" else (path_flags(pdm, path) | (csize << pdm.PDM_CTAS_SHIFT))
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        ref = plan.migrate(p0).clone()
+        img = torch.empty_like(ref)
+        for _ in range(60):
+            plan.migrate(p0, img)
+            assert torch.equal(img, ref), name
+    assert torch.isfinite(ref).all()
+
+
 def test_repeated_migrate_is_bit_identical_and_plans_are_independent(pdm):
     import torch
     a = pdm_inputs.random_problem(21, 700, 20, 300, 15, model="field")
