@@ -39,7 +39,10 @@ typedef enum {
                                       symmetric taps (W_k == W_-k, north_star) and would silently
                                       compute something else                                       */
     PDM_ERR_UNSUPPORTED = -4,      /* not a CC 10.x device; forced path impossible for this nx;
-                                      ntaps above PDM_MAX_TAPS                                     */
+                                      ntaps above PDM_MAX_TAPS; a forced SMEM / TILED / CLUSTER path
+                                      with more than 51 taps (the longest unrolled kernel; shorter
+                                      filters of any odd length run on the next longer kernel with
+                                      zero taps appended, longer ones only on PDM_PATH_NAIVE)      */
     PDM_ERR_NOMEM = -5,            /* host or device allocation failed                             */
     PDM_ERR_CUDA = -6              /* a CUDA call failed; pdm_info.last_cuda_error has the code    */
 } pdm_status;

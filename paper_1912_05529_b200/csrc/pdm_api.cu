@@ -147,8 +147,18 @@ static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false, int 
 }
 static cluster_fn cluster_kernel_for(int L, bool taps_smem) { return pdm_cluster_kernel_for(L, taps_smem); }
 // output tile aliased onto the consumed input tile: only where it pays (long per-sample rows)
-static bool tiled_alias(const pdm_plan *p) { return p->contiguous_rows != 0 && p->L == 25; }
-static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide) { return pdm_tiled_kernel_for(p->L, wide, tiled_alias(p)); }
+static bool tiled_alias(const pdm_plan *p) { return p->contiguous_rows != 0 && p->Lk == 25; }
+static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide) { return pdm_tiled_kernel_for(p->Lk, wide, tiled_alias(p)); }
+// Filter lengths without an instantiation of their own run on the next longer one with the extra
+// taps set to zero (x + 0*s == x exactly), so every odd length up to the longest instantiation
+// takes the unrolled kernels; 0 = longer than all of them (scaffold only).
+static int kernel_half_length(int L)
+{
+#define X(LL) if (L <= LL) return LL;
+    PDM_FOR_EACH_L(X)
+#undef X
+    return 0;
+}
 // Work list of the marching kernel.  Unbalanced: CTA c owns whole lines c, c+grid, ...  Balanced
 // (nw >= grid): the nw*nz depth steps, laid end to end line after line, are cut into `grid` equal
 // ranges; a range is [tail of a line][whole lines][head of a line].  The CTA runs its head FIRST
@@ -191,7 +201,7 @@ static void build_segments(int nw, int nz, int grid, bool balance,
 // Row de-duplication inside a thread (pdm_fir_group DEDUP) pays where nearly every sample has its
 // own table row and the filter is short enough to leave registers: measured +4..7 % on the marching
 // path for taps <= 35 on random-field models, -4 % at 51 taps, -10 % on the 128-register tiled kernel.
-static bool use_dedup(const pdm_plan *p) { return p->contiguous_rows != 0 && p->L <= 17; }
+static bool use_dedup(const pdm_plan *p) { return p->contiguous_rows != 0 && p->Lk <= 17; }
 
 static int halo_groups(int L, int R) { return (L + 1 + R - 1) / R; }
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
@@ -199,6 +209,8 @@ static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 static int build_plan(pdm_plan *p, const float *omega, const float *velocity, const pdm_c64 *table)
 {
     const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, ntaps = p->ntaps, L = p->L;
+    const int Lk = kernel_half_length(L);                  // 0: no unrolled kernel is long enough
+    p->Lk = Lk;
     // outputs per thread: 8, or 4 for short lines with so few of them that 8 would leave the SMs
     // with under 8 warps each (configs[0], [1]); only the single-CTA marching form has the R = 4 build
     const unsigned want_path = p->flags & PDM_PATH_MASK;
@@ -230,7 +242,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     }
 
     // ---- half table: rows k = 0..L as float4 pairs (W_2t, W_2t+1), odd number of float4 per row
-    p->half16 = ((L + 2) / 2) | 1;
+    p->half16 = ((std::max(L, Lk) + 2) / 2) | 1;            // rows padded with zero taps up to Lk
     std::vector<float4> half((size_t)ntab * p->half16, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int j = 0; j < ntab; ++j)
         for (int k = 0; k <= L; ++k) {
@@ -283,8 +295,8 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     // ---- choose the kernel form ----------------------------------------------------------------------
     const unsigned want = p->flags & PDM_PATH_MASK;
     const unsigned want_taps = p->flags & PDM_TAPS_MASK;
-    const bool have_L = march_kernel_for(L, false) != nullptr;
-    const int HG = halo_groups(L, R);
+    const bool have_L = Lk != 0;
+    const int HG = halo_groups(have_L ? Lk : L, R);
     const int ngroups = (nx + R - 1) / R;
     const int slots = (2 * HG + ngroups) * (R + 2);
     const int map_len = round_up(ntab, 8);
@@ -350,7 +362,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         }
         p->threads = threads;
         p->smem_bytes = (int)(line_bytes + (p->taps_in_smem ? slice_bytes : 0));
-        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0, use_dedup(p), R);
+        march_fn fn = march_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p), R);
         PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          p->smem_bytes));
         int per_sm = 0;
@@ -394,7 +406,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->threads = 32 * nwarps;
         p->cluster_size = C; p->cluster_gper = gper; p->cluster_passes = passes;
         p->smem_bytes = (int)(seg_bytes + (p->taps_in_smem ? slice_bytes : 0));
-        cluster_fn fn = cluster_kernel_for(L, p->taps_in_smem != 0);
+        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0);
         PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          p->smem_bytes));
         int max_clusters = 0;
@@ -468,7 +480,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
     PDM_CUDA(p, cudaGetDevice(&dev));
     if (dev != p->device) { p->last_cuda_error = (int)cudaErrorInvalidDevice; return PDM_ERR_CUDA; }
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const int nx = p->nx, nz = p->nz, nw = p->nw, L = p->L, R = p->R;
+    const int nx = p->nx, nz = p->nz, nw = p->nw, L = p->L, Lk = p->Lk, R = p->R;
     const float2 *P0 = reinterpret_cast<const float2 *>(P0_dev);
 
     if (p->path == PDM_PATH_SMEM) {
@@ -480,9 +492,9 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.ngroups = (nx + R - 1) / R;
         a.qstride = p->qstride; a.pstride = a.ngroups * R; a.half16 = p->half16;
         a.passes = (a.ngroups + p->threads - 1) / p->threads;
-        a.slots = (2 * halo_groups(L, R) + a.ngroups) * (R + 2);
+        a.slots = (2 * halo_groups(Lk, R) + a.ngroups) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
-        march_fn fn = march_kernel_for(L, p->taps_in_smem != 0, use_dedup(p), R);
+        march_fn fn = march_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p), R);
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
         if (p->balanced) {                               // split lines: CTAs wait on one another
             void *args[] = { (void *)&a };
@@ -504,10 +516,10 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.ngroups = (nx + R - 1) / R;
         a.qstride = p->qstride; a.pstride = a.ngroups * R; a.half16 = p->half16;
         a.passes = p->cluster_passes; a.gper = p->cluster_gper;
-        a.slots = (2 * halo_groups(L, R) + a.gper) * (R + 2);
+        a.slots = (2 * halo_groups(Lk, R) + a.gper) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
         a.nclusters = p->n_partial;
-        cluster_fn fn = cluster_kernel_for(L, p->taps_in_smem != 0);
+        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0);
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
@@ -616,7 +628,7 @@ extern "C" int pdm_get_info(const pdm_plan *p, pdm_info *out)
     out->sm_count = p->sm_count; out->last_cuda_error = p->last_cuda_error;
     out->samples = (double)p->nx * (double)p->nz * (double)p->nw;
     out->counted_flops = 8.0 * p->ntaps * out->samples;
-    out->executed_lane_ops = (6.0 * p->L + 4.0) * out->samples;
+    out->executed_lane_ops = (6.0 * (p->Lk ? p->Lk : p->L) + 4.0) * out->samples;   // zero-padded taps are executed too
     out->workspace_bytes = p->workspace_bytes;
     return PDM_OK;
 }

@@ -9,6 +9,7 @@
 
 struct pdm_plan {
     int nx, nz, nw, ntab, ntaps, L;
+    int Lk;               // half-length of the unrolled kernel instantiation used (>= L; taps beyond L are zero)
     float dx, dz;
     double du;
     unsigned flags;

@@ -88,8 +88,16 @@ def test_short_filters_and_tiny_grids(pdm, path, L):
         assert_parity(pdm, cfg, path_flags(pdm, path))
 
 
-def test_filter_length_without_unrolled_kernel_uses_scaffold(pdm):
-    cfg = pdm_inputs.tiny_random_problem(7, nx=40, nz=6, nw=3, L=5, ntab=11)   # 11 taps: no instantiation
+def test_filter_lengths_without_their_own_unrolled_kernel(pdm):
+    """Lengths between two instantiations run on the next longer one with zero taps appended (every
+    kernel form); lengths beyond the longest fall back to the scaffold."""
+    for L, nx in ((5, 40), (10, 333), (20, 1200), (24, 2600)):     # -> kernels for L = 7, 12, 25, 25
+        cfg = pdm_inputs.tiny_random_problem(7 + L, nx=nx, nz=6, nw=3, L=L, ntab=11)
+        ref = oracle.migrate(cfg)
+        assert_parity(pdm, cfg, 0, ref=ref, expect_path=pdm.PDM_PATH_SMEM)
+        for path in ("smem_global", "tiled", "cluster"):
+            assert_parity(pdm, cfg, path_flags(pdm, path), ref=ref)
+    cfg = pdm_inputs.tiny_random_problem(9, nx=50, nz=4, nw=2, L=30, ntab=9)   # 61 taps: longer than any
     assert_parity(pdm, cfg, 0, expect_path=pdm.PDM_PATH_NAIVE)
     rc, h = pdm.pdm_create(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"],
                            cfg["velocity"], cfg["table"], cfg["du"], pdm.PDM_PATH_SMEM)
