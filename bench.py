@@ -329,9 +329,12 @@ def run_sweep(args):
     torch.cuda.set_device(dev)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    with open("/root/repo/MEASURED_PEAKS.json") if os.path.exists("/root/repo/MEASURED_PEAKS.json") \
-            else open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
-        hbm_gbs = json.load(f)["hbm_gbs"]
+    hbm_gbs, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"    # used only if the driver's file is absent
+    for cand in ("/root/repo/MEASURED_PEAKS.json", os.path.join(ROOT, "MEASURED_PEAKS.json")):
+        if os.path.exists(cand):
+            with open(cand) as f:
+                hbm_gbs, hbm_src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+            break
     def pick(arg, full):
         return tuple(int(t) for t in arg.split(",")) if arg else full
     for ntaps in pick(args.sweep_taps, SWEEP_TAPS):
@@ -364,7 +367,8 @@ def run_sweep(args):
                        "launches": info["launches_per_migrate"], "steps": steps, "ms": t * 1e3,
                        "samples_per_s": sps,
                        "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
-                       "frac_hbm_16B_per_sample": (sps * 16 / (hbm_gbs * 1e9)) if tiled else None}
+                       "frac_hbm_16B_per_sample": (sps * 16 / (hbm_gbs * 1e9)) if tiled else None,
+                       "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src}
                 print(json.dumps(out), flush=True)
                 plan.close()
                 del P0, image

@@ -497,6 +497,8 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         march_fn fn = march_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p), R);
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
         if (p->balanced) {                               // split lines: CTAs wait on one another
+            // hand-off flags start empty even if an earlier migrate on this plan was cut short
+            PDM_CUDA(p, cudaMemsetAsync(p->d_flags, 0, (size_t)std::max(1, p->nslots) * sizeof(int), st));
             void *args[] = { (void *)&a };
             PDM_CUDA(p, cudaLaunchCooperativeKernel((const void *)fn, dim3(p->grid), dim3(p->threads),
                                                     args, (size_t)p->smem_bytes, st));
