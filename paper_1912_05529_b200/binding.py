@@ -271,6 +271,14 @@ class Plan:
             raise PdmError(rc, "pdm_migrate")
         return image
 
+    def migrate_section(self, transform: "SectionTransform", section, image=None, stream=None):
+        """t-x section (cuda float32 [nt][nx]) -> image: pdm_tf_forward then pdm_migrate, both
+        enqueued on one stream (marshalling only; P0 is the unscaled transform)."""
+        import torch
+        st = stream or torch.cuda.current_stream(section.device)
+        P0 = transform.forward(section, stream=st)
+        return self.migrate(P0, image, stream=st)
+
     def migrate_host(self, P0_host, image_host=None, stream=None):
         """End-to-end call: HOST complex64 [nw, nx] (numpy or pinned torch) -> HOST float32 [nz, nx]."""
         import torch

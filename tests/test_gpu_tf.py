@@ -88,7 +88,7 @@ def test_section_to_image_end_to_end(pdm):
     omega = (2 * np.pi * bins / (nt * dt)).astype(np.float32)
     rng = np.random.default_rng(4)
     section = rng.standard_normal((nt, cfg["nx"])).astype(np.float32)
-    scale = 1.0 / np.sqrt(nt)
+    scale = 1.0                                            # P0 is the unscaled transform
     # frequencies of the record's own bins; the table abscissa must still cover omega*q
     cfg = dict(cfg, omega=omega, nw=bins.size,
                du=float(omega.max() * cfg["dz"] / cfg["velocity"].min() / (cfg["ntab"] - 1)))
@@ -99,6 +99,9 @@ def test_section_to_image_end_to_end(pdm):
         img = plan.migrate(P0.contiguous())
         torch.cuda.synchronize()
         got = img.cpu().numpy().astype(np.float64)
+        img2 = plan.migrate_section(tf, torch.from_numpy(section).cuda())               # one-call form
+        torch.cuda.synchronize()
+        assert np.array_equal(img2.cpu().numpy(), img.cpu().numpy())
     rel = np.linalg.norm(got - ref) / np.linalg.norm(ref)
     mx = np.abs(got - ref).max() / np.abs(ref).max()
     assert rel <= 1e-4 and mx <= 1e-3, (rel, mx)
