@@ -332,11 +332,20 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     // 1.3-1.8x on configs[4] nw = 64 points with nx >= 4096) and the tap rows can still be staged
     const bool auto_cluster = cl_slice_ok && 2 * nw <= p->sm_count && ngroups >= 512 &&
                               (long long)nw * cl_C <= 2LL * p->sm_count;
+    // ... and for lines that do not fit one CTA but do fit a PAIR (nx = 16384 with 51 taps or fewer),
+    // when the tap rows can be staged and the lines fill the clusters' rounds: the wavefield then never
+    // touches HBM (measured 1.05-1.2x over the x-tiled form at nw >= 1024; larger clusters lose SMs to
+    // GPC fragmentation and stay with the x-tiled form)
+    bool auto_pair = false;
+    if (!lines_fit && cl_C == 2 && cl_slice_ok) {
+        const int ncl = std::max(1, p->sm_count / 2);
+        auto_pair = (double)nw / ((double)ncl * ((nw + ncl - 1) / ncl)) >= 0.95;
+    }
     if (want == PDM_PATH_CLUSTER && !cl_C) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;  // (tiled_kernel_for has the same L list)
     if (want == PDM_PATH_AUTO)
-        p->path = auto_cluster ? PDM_PATH_CLUSTER
+        p->path = (auto_cluster || auto_pair) ? PDM_PATH_CLUSTER
                                : (lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE));
     else p->path = (int)want;
 
