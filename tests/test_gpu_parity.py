@@ -234,6 +234,15 @@ def _subset_parity(pdm, cfg, lines, flags=0, expect_path=None):
 
 
 @pytest.mark.slow
+def test_config3_full_image_in_the_bench_configuration(pdm):
+    """The whole configs[3] image (6144 x 1500, all 803 frequencies), in the launch configuration
+    bench.py times (AUTO: balanced SMEM marching), against the full FP64 oracle run."""
+    cfg = pdm_inputs.make_config(3)
+    rel, mx = assert_parity(pdm, cfg, 0, expect_path=pdm.PDM_PATH_SMEM)
+    assert rel <= 1e-5 and mx <= 1e-5, (rel, mx)          # measured ~1.5e-6: well inside the 1e-4 bar
+
+
+@pytest.mark.slow
 def test_config3_full_size_sampled_frequencies(pdm):
     cfg = pdm_inputs.make_config(3)
     nw = cfg["nw"]
