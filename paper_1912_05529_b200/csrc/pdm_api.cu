@@ -339,7 +339,9 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     bool auto_pair = false;
     if (!lines_fit && cl_C == 2 && cl_slice_ok) {
         const int ncl = std::max(1, p->sm_count / 2);
-        auto_pair = (double)nw / ((double)ncl * ((nw + ncl - 1) / ncl)) >= 0.95;
+        // per-sample-row models gain 1.19x from the pair at full rounds, warp-uniform ones nothing:
+        // the former may waste up to 15 % of the last round and still win
+        auto_pair = (double)nw / ((double)ncl * ((nw + ncl - 1) / ncl)) >= (p->contiguous_rows ? 0.85 : 0.95);
     }
     if (want == PDM_PATH_CLUSTER && !cl_C) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
