@@ -33,6 +33,7 @@ struct pdm_march_params {
     const float4 *half;      // [ntab][half16]
     const int    *rowoff;    // [nw+1]
     const int    *rows;      // row lists
+    cudaTextureObject_t tex; // the half table as a linear float4 texture
     const int4   *segs;      // work list: {line, z0, z1, hand-off slot or -1}, in execution order per CTA
     const int    *segoff;    // [grid+1] offsets into segs
     float2       *handoff;   // [nslots][nx] wavefield of a line split between two CTAs, at the split depth
@@ -58,13 +59,27 @@ __device__ __forceinline__ float2 f4hi(float4 v) { return make_float2(v.z, v.w);
 // packed operand and the folded sample as the scalar one: the tap pair is then the same register
 // pair for up to 2R consecutive FFMA2 (register-reuse cache), which keeps the register-file reads
 // per instruction at <= 2 per bank; the scalar-tap form measured 0.80 of the pipe at best.
-template <int L, int R, bool UNIFORM, bool DEDUP>
+// TEXMASK: bit r set = output r fetches its tap rows through the TEXTURE unit (tex1Dfetch on the
+// global half table; toff[r] is then a GLOBAL float4 index) through a 3-deep register ring, instead
+// of the LSU path: the texture unit is a second gather path whose bandwidth adds to the LSU's
+// (random 16-byte gathers, measured: shared memory 54 B/clk/SM, texture 23, mixed 3:1 71).
+template <int L, int R, bool UNIFORM, bool DEDUP, unsigned TEXMASK = 0u>
 __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
                                               const float4 *__restrict__ tbase,
-                                              const int (&toff)[R], float2 (&out)[R])
+                                              const int (&toff)[R], float2 (&out)[R],
+                                              cudaTextureObject_t tex = 0)
 {
     float2 wl[R], wr[R], acc_a[R], acc_b[R];
     float4 tw[UNIFORM ? 1 : R];
+    constexpr int TMAX = L / 2;                         // last float4 of a half row that is used
+    float4 tx[R][3];
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if ((TEXMASK >> r) & 1u) {
+#pragma unroll
+            for (int s = 0; s < 3; ++s)
+                if (s <= TMAX) tx[r][s] = tex1Dfetch<float4>(tex, toff[r] + s);
+        }
 #pragma unroll
     for (int i = 0; i < R / 2; ++i) {
         const float4 v = *reinterpret_cast<const float4 *>(base + 2 * i);
@@ -76,7 +91,8 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
     // fetching a row only where it differs from the previous output's (predicated loads) pays.
     bool same[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) same[r] = DEDUP && !UNIFORM && r > 0 && toff[r] == toff[r - 1];
+    for (int r = 0; r < R; ++r)
+        same[r] = ((TEXMASK >> r) & 1u) || (DEDUP && !UNIFORM && r > 0 && !((TEXMASK >> (r - 1)) & 1u) && toff[r] == toff[r - 1]);
 #pragma unroll
     for (int r = 0; r < (UNIFORM ? 1 : R); ++r) {
         if (DEDUP && r > 0) tw[r] = tw[r - 1];
@@ -84,7 +100,7 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
     }
 #pragma unroll
     for (int r = 0; r < R; ++r) {                       // centre tap W_0
-        const float4 t = tw[UNIFORM ? 0 : r];
+        const float4 t = ((TEXMASK >> r) & 1u) ? tx[r][0] : tw[UNIFORM ? 0 : r];
         acc_a[r] = pk_mul_s(wl[r].x, f4lo(t));
         acc_b[r] = pk_mul_s(wl[r].y, f4lo(t));
     }
@@ -107,11 +123,16 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
         }
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            const float4 t = tw[UNIFORM ? 0 : r];
+            const float4 t = ((TEXMASK >> r) & 1u) ? tx[r][(k / 2) % 3] : tw[UNIFORM ? 0 : r];
             const float2 W = (k & 1) ? f4hi(t) : f4lo(t);
             const float2 s = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
             acc_a[r] = pk_fma_s(s.x, W, acc_a[r]);
             acc_b[r] = pk_fma_s(s.y, W, acc_b[r]);
+        }
+        if ((k & 1) && k / 2 + 3 <= TMAX) {             // float4 k/2 is spent: refill its ring slot
+#pragma unroll
+            for (int r = 0; r < R; ++r)
+                if ((TEXMASK >> r) & 1u) tx[r][(k / 2) % 3] = tex1Dfetch<float4>(tex, toff[r] + k / 2 + 3);
         }
     }
 #pragma unroll
@@ -126,6 +147,9 @@ __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ?
     static_assert(R % 2 == 0 && R >= 2, "R must be even");
     constexpr int HG = pdm_halo_groups<L, R>();
     constexpr int GS = R + 2;
+    // per-sample-row plans only: 2 of a thread's 8 tap rows through the texture unit for the shortest
+    // filters, 1 of 8 for longer ones (measured best per length; more costs registers the loop needs)
+    constexpr unsigned TEXMASK = (DEDUP && R == 8) ? (L <= 7 ? 0x88u : 0x80u) : 0u;
     extern __shared__ __align__(16) unsigned char pdm_smem[];
     float2 *buf_a = reinterpret_cast<float2 *>(pdm_smem);
     float2 *buf_b = buf_a + p.slots;
@@ -228,7 +252,8 @@ __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ?
                 }
                 un = u;
 #pragma unroll
-                for (int r = 0; r < R; ++r) tn[r] = (TAPS_SMEM ? (int)map[jn[r]] : jn[r]) * p.half16;
+                for (int r = 0; r < R; ++r)
+                    tn[r] = (((TEXMASK >> r) & 1u) ? jn[r] : (TAPS_SMEM ? (int)map[jn[r]] : jn[r])) * p.half16;
             };
             load_q(z0, 0);
             index_next();
@@ -274,7 +299,7 @@ __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ?
                     const float2 *base = cur + (HG + g) * GS;
                     float2 out[R];
                     if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
-                    else     pdm_fir_group<L, R, false, DEDUP>(base, tbase, toff, out);
+                    else     pdm_fir_group<L, R, false, DEDUP, TEXMASK>(base, tbase, toff, out, p.tex);
                     if (active) {
                         const int x0 = g * R;
                         float2 *dst = nxt + (HG + g) * GS;

@@ -54,6 +54,7 @@ static inline int host_index(float w, float q, int ntab)
 static void free_plan(pdm_plan *p)
 {
     if (!p) return;
+    if (p->tex_half) cudaDestroyTextureObject(p->tex_half);
     cudaFree(p->d_omega); cudaFree(p->d_q); cudaFree(p->d_table); cudaFree(p->d_half);
     cudaFree(p->d_rowoff); cudaFree(p->d_rows); cudaFree(p->d_partial);
     cudaFree(p->d_plane[0]); cudaFree(p->d_plane[1]); cudaFree(p->d_flags);
@@ -404,6 +405,15 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->n_partial * nz * (ngroups * R))) != PDM_OK) return rc;
+        {
+            cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
+            rd.resType = cudaResourceTypeLinear; rd.res.linear.devPtr = p->d_half;
+            rd.res.linear.desc = cudaCreateChannelDesc<float4>();
+            rd.res.linear.sizeInBytes = half.size() * sizeof(float4);
+            cudaTextureDesc td; memset(&td, 0, sizeof(td));
+            td.readMode = cudaReadModeElementType;
+            PDM_CUDA(p, cudaCreateTextureObject(&p->tex_half, &rd, &td, nullptr));
+        }
     } else if (p->path == PDM_PATH_CLUSTER) {
         const int C = cl_C, passes = cl_passes, nwarps = cl_nwarps, gper = cl_gper;
         const size_t seg_bytes = cl_seg_bytes;
@@ -497,7 +507,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
     if (p->path == PDM_PATH_SMEM) {
         pdm_march_params a;
         a.P0 = P0; a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega;
-        a.half = p->d_half; a.rowoff = p->d_rowoff; a.rows = p->d_rows;
+        a.half = p->d_half; a.rowoff = p->d_rowoff; a.rows = p->d_rows; a.tex = p->tex_half;
         a.segs = p->d_segs; a.segoff = p->d_segoff; a.handoff = p->d_handoff; a.flags = p->d_flags;
         a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
         a.ngroups = (nx + R - 1) / R;

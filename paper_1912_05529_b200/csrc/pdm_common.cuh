@@ -22,6 +22,7 @@ struct pdm_plan {
     float  *d_q;          // [nz][qstride]  q32 = fl32(dz/(v*du)) (R3); columns >= nx repeat the last q
     int     qstride;      // row stride of d_q (multiple of 32 floats)
     float2 *d_table;      // full table [ntab][ntaps] (naive path only reads this)
+    cudaTextureObject_t tex_half;   // d_half as a linear float4 texture (tap gather through the texture unit)
     float4 *d_half;       // half table rows k=0..L as (W_k, W_{k+1}) pairs, [ntab][half16] float4
     int     half16;       // float4 per row, odd
     int    *d_rowoff;     // [nw+1] offsets into d_rows
