@@ -28,17 +28,21 @@ struct pdm_cluster_params {
     const float4 *half;      // [ntab][half16]
     const int    *rowoff;    // [nw+1]
     const int    *rows;      // row lists
+    cudaTextureObject_t tex; // the half table as a linear float4 texture
     int nx, nz, nw, ntab;
     int qstride, pstride, half16;
     int ngroups, passes, gper, slots, map_len, nclusters;
 };
 
-template <int L, int R, bool TAPS_SMEM>
+template <int L, int R, bool TAPS_SMEM, bool DEDUP>
 __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(const pdm_cluster_params p)
 {
     namespace cg = cooperative_groups;
     constexpr int HG = pdm_halo_groups<L, R>();
     constexpr int GS = R + 2;
+    // per-sample-row plans: row de-duplication and part of the tap gather through the texture unit,
+    // exactly as in pdm_march_kernel
+    constexpr unsigned TEXMASK = DEDUP ? (L <= 7 ? 0x88u : 0x80u) : 0u;
     cg::cluster_group cluster = cg::this_cluster();
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
     const int cid = blockIdx.x / C;
@@ -123,7 +127,8 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(c
                 }
                 un = u;
 #pragma unroll
-                for (int r = 0; r < R; ++r) tn[r] = (TAPS_SMEM ? (int)map[jn[r]] : jn[r]) * p.half16;
+                for (int r = 0; r < R; ++r)
+                    tn[r] = (((TEXMASK >> r) & 1u) ? jn[r] : (TAPS_SMEM ? (int)map[jn[r]] : jn[r])) * p.half16;
             };
             load_q(0, 0);
             index_next();
@@ -166,7 +171,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(c
                     const float2 *base = cur + (HG + gl) * GS;
                     float2 out[R];
                     if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
-                    else     pdm_fir_group<L, R, false, false>(base, tbase, toff, out);
+                    else     pdm_fir_group<L, R, false, DEDUP, TEXMASK>(base, tbase, toff, out, p.tex);
                     if (active) {
                         const int x0 = g * R;
                         float2 *dst = nxt + (HG + gl) * GS;

@@ -146,7 +146,7 @@ static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false, int 
     if (!f) f = pdm_march_kernel_part2(L, taps_smem, dedup, R);
     return f;
 }
-static cluster_fn cluster_kernel_for(int L, bool taps_smem) { return pdm_cluster_kernel_for(L, taps_smem); }
+static cluster_fn cluster_kernel_for(int L, bool taps_smem, bool dedup) { return pdm_cluster_kernel_for(L, taps_smem, dedup); }
 // output tile aliased onto the consumed input tile: only where it pays (long per-sample rows)
 static bool tiled_alias(const pdm_plan *p) { return p->contiguous_rows != 0 && p->Lk == 25; }
 static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide) { return pdm_tiled_kernel_for(p->Lk, wide, tiled_alias(p)); }
@@ -203,6 +203,20 @@ static void build_segments(int nw, int nz, int grid, bool balance,
 // own table row and the filter is short enough to leave registers: measured +4..7 % on the marching
 // path for taps <= 35 on random-field models, -4 % at 51 taps, -10 % on the 128-register tiled kernel.
 static bool use_dedup(const pdm_plan *p) { return p->contiguous_rows != 0 && p->Lk <= 17; }
+
+// the half table as a linear float4 texture: the per-sample-row kernel variants fetch part of their
+// tap rows through the texture unit (a second gather path next to the LSU)
+static int make_half_texture(pdm_plan *p, size_t count)
+{
+    cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
+    rd.resType = cudaResourceTypeLinear; rd.res.linear.devPtr = p->d_half;
+    rd.res.linear.desc = cudaCreateChannelDesc<float4>();
+    rd.res.linear.sizeInBytes = count * sizeof(float4);
+    cudaTextureDesc td; memset(&td, 0, sizeof(td));
+    td.readMode = cudaReadModeElementType;
+    PDM_CUDA(p, cudaCreateTextureObject(&p->tex_half, &rd, &td, nullptr));
+    return PDM_OK;
+}
 
 static int halo_groups(int L, int R) { return (L + 1 + R - 1) / R; }
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
@@ -405,15 +419,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->n_partial * nz * (ngroups * R))) != PDM_OK) return rc;
-        {
-            cudaResourceDesc rd; memset(&rd, 0, sizeof(rd));
-            rd.resType = cudaResourceTypeLinear; rd.res.linear.devPtr = p->d_half;
-            rd.res.linear.desc = cudaCreateChannelDesc<float4>();
-            rd.res.linear.sizeInBytes = half.size() * sizeof(float4);
-            cudaTextureDesc td; memset(&td, 0, sizeof(td));
-            td.readMode = cudaReadModeElementType;
-            PDM_CUDA(p, cudaCreateTextureObject(&p->tex_half, &rd, &td, nullptr));
-        }
+        if ((rc = make_half_texture(p, half.size())) != PDM_OK) return rc;
     } else if (p->path == PDM_PATH_CLUSTER) {
         const int C = cl_C, passes = cl_passes, nwarps = cl_nwarps, gper = cl_gper;
         const size_t seg_bytes = cl_seg_bytes;
@@ -427,7 +433,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->threads = 32 * nwarps;
         p->cluster_size = C; p->cluster_gper = gper; p->cluster_passes = passes;
         p->smem_bytes = (int)(seg_bytes + (p->taps_in_smem ? slice_bytes : 0));
-        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0);
+        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p));
         PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          p->smem_bytes));
         int max_clusters = 0;
@@ -449,6 +455,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if ((rc = dev_upload(p, &p->d_rowoff, rowoff.data(), rowoff.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_rows, rows.data(), rows.size())) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->n_partial * nz * (ngroups * R))) != PDM_OK) return rc;
+        if ((rc = make_half_texture(p, half.size())) != PDM_OK) return rc;
     } else if (p->path == PDM_PATH_TILED) {
         p->taps_mode = 1;
         p->threads = PDM_TILED_THREADS;
@@ -542,7 +549,8 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.slots = (2 * halo_groups(Lk, R) + a.gper) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
         a.nclusters = p->n_partial;
-        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0);
+        a.tex = p->tex_half;
+        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p));
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;

@@ -22,5 +22,5 @@ typedef void (*cluster_fn)(const pdm_cluster_params);
 march_fn pdm_march_kernel_part0(int L, bool taps_smem, bool dedup, int R);
 march_fn pdm_march_kernel_part1(int L, bool taps_smem, bool dedup, int R);
 march_fn pdm_march_kernel_part2(int L, bool taps_smem, bool dedup, int R);
-cluster_fn pdm_cluster_kernel_for(int L, bool taps_smem);
+cluster_fn pdm_cluster_kernel_for(int L, bool taps_smem, bool dedup);
 tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias);
