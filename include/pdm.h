@@ -50,13 +50,16 @@ typedef enum {
 #define PDM_MAX_TAPS 129           /* L <= 64 */
 
 /* flags word of pdm_create: bits 0-3 choose the kernel form, the rest are tuning/debug knobs.     */
-#define PDM_PATH_AUTO    0u  /* SMEM marching if a line (ping-pong) fits one CTA, else x-tiled      */
+#define PDM_PATH_AUTO    0u  /* SMEM marching if a line (ping-pong) fits one CTA, else x-tiled; the  */
+                             /* cluster form when there are too few lines to fill the SMs, or when a */
+                             /* line fits a pair of CTAs and its tap rows can still be staged        */
 #define PDM_PATH_SMEM    1u  /* main form: one CTA keeps a frequency's x-line in shared memory and   */
                              /* marches all nz depth steps in place (north_star)       */
 #define PDM_PATH_TILED   2u  /* x-tiled per-depth-step kernel with +-L halos, planes ping-pong in HBM*/
 #define PDM_PATH_NAIVE   3u  /* scaffold: one thread per (w,x) sample, one launch per depth level --  */
                              /* the paper's own mapping, kept only as a cross-check    */
-#define PDM_PATH_CLUSTER 4u  /* line split over a thread-block cluster with DSMEM halos              */
+#define PDM_PATH_CLUSTER 4u  /* main form with the line split over a thread-block cluster of 2, 4 or */
+                             /* 8 CTAs, halos exchanged through distributed shared memory            */
 #define PDM_PATH_MASK    0xFu
 #define PDM_TAPS_AUTO    (0u << 4)  /* where the kernels read filter rows from                      */
 #define PDM_TAPS_GLOBAL  (1u << 4)  /* always from the L2/L1-cached global half-table               */
@@ -66,7 +69,8 @@ typedef enum {
 #define PDM_FORCE_GENERAL (1u << 6) /* debug: never take the uniform-index fast path                */
 #define PDM_NO_BALANCE   (1u << 7)  /* debug: whole lines per CTA (no depth-split load balancing)   */
 #define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto)                   */
-#define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto)   */
+#define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
+                                    /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
 #define PDM_TILE_SHIFT    20        /* bits 20-27: x-tile size / 256 samples for PDM_PATH_TILED     */
 #define PDM_FLAGS_VALID  0x0FFFFFFFu
 
