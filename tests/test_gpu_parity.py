@@ -199,6 +199,21 @@ def test_cluster_path_matches_oracle(pdm, nx, nz, nw, ntaps, model, csize):
     assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
 
 
+def test_auto_policy_picks_the_measured_best_form(pdm):
+    """pdm_create's AUTO choice (flags = 0) for the regimes measured in profiles/r01_sweep_config4.md."""
+    def path_of(nx, nw, ntaps, model):
+        cfg = pdm_inputs.random_problem(71, nx, 4, nw, ntaps, model=model)
+        with pdm.Plan.from_config(cfg, 0) as plan:
+            return plan.info
+    assert path_of(2048, 300, 25, "layers")["path"] == pdm.PDM_PATH_SMEM        # plenty of lines
+    small = path_of(512, 100, 31, "layers")                                     # few short lines: R = 4
+    assert small["path"] == pdm.PDM_PATH_SMEM and small["threads_per_cta"] == 128
+    assert path_of(4096, 40, 25, "layers")["path"] == pdm.PDM_PATH_CLUSTER      # too few lines for 148 SMs
+    assert path_of(16384, 592, 15, "layers")["path"] == pdm.PDM_PATH_CLUSTER    # a line fits a pair of CTAs
+    assert path_of(16384, 200, 15, "layers")["path"] == pdm.PDM_PATH_TILED      # ... but 200 lines waste a round
+    assert path_of(32768, 400, 15, "layers")["path"] == pdm.PDM_PATH_TILED      # north_star: forced x-tiled
+
+
 # ---------------------------------------------------------------- BASELINE.json configs
 def test_config0_all_paths(pdm, config0):
     ref = oracle.migrate(config0)
