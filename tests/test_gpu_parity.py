@@ -278,6 +278,32 @@ def test_config4_points_sampled_frequencies(pdm, nx, nw, ntaps):
         _subset_parity(pdm, cfg, lines, pdm.PDM_PATH_TILED, expect_path=pdm.PDM_PATH_TILED)
 
 
+@pytest.mark.slow
+def test_randomized_parity_over_forms_shapes_and_filter_lengths(pdm):
+    """Seeded fuzz: random (nx, nz, nw, taps, model, kernel form) -- ragged sizes around the 8-sample
+    group and the 32-group warp, filter lengths with and without their own instantiation, every
+    cluster size -- each against the oracle at the north_star bar."""
+    import torch
+    rng = np.random.default_rng(2024)
+    forms = [0, pdm.PDM_PATH_SMEM, pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_GLOBAL, pdm.PDM_PATH_TILED,
+             pdm.PDM_PATH_CLUSTER, pdm.PDM_PATH_CLUSTER | (4 << pdm.PDM_CTAS_SHIFT),
+             pdm.PDM_PATH_CLUSTER | (8 << pdm.PDM_CTAS_SHIFT)]
+    for i in range(48):
+        nx = int(rng.choice([1, 7, 8, 9, 63, 64, 65, 255, 257, 700, 1023, 1500, 2049, 3333, 5000]))
+        nz = int(rng.integers(1, 24))
+        nw = int(rng.choice([1, 2, 5, 37, 150, 310]))
+        ntaps = int(rng.choice([3, 5, 7, 9, 11, 15, 21, 25, 31, 35, 41, 51]))
+        model = str(rng.choice(["field", "white", "layers", "const"]))
+        flags = int(rng.choice(forms))
+        if nx * nz * nw > 4e6:
+            nw = max(1, int(4e6 // (nx * nz)))
+        cfg = pdm_inputs.random_problem(1000 + i, nx, nz, nw, ntaps, model=model)
+        img = gpu_migrate(pdm, cfg, flags)
+        rel, mx = errors(img, oracle.migrate(cfg))
+        assert np.isfinite(img).all() and rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, \
+            (i, nx, nz, nw, ntaps, model, hex(flags), rel, mx)
+
+
 # ---------------------------------------------------------------- properties of the GPU path itself
 def test_delta_table_is_identity_on_gpu(pdm):
     cfg = pdm_inputs.random_problem(3, 520, 9, 4, 25, model="field")
