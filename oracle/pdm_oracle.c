@@ -38,9 +38,12 @@
  * Pins (tests/test_oracle_pins.py, all `-m "not gpu"`): P1 delta table = identity, P2 brute
  * force on tiny grids, P3 spectral identity, P4 exact phase shift in constant velocity,
  * P5 point-diffractor focusing, P7 superposition, P8 w-additivity/permutation, P9 mirror,
- * P10 energy non-growth, P11 shift invariance, P12 index rule.  Parity unpinned by anything
- * external: the choices R5/R6/R7 (boundary, row<->depth, velocity row) and the absolute
- * amplitude scale R10 -- fixed by DESIGN.md only.
+ * P10 energy non-growth, P11 shift invariance, P12a index rule (the function), P12b index rule
+ * THROUGH the migrate loop (centre-tap-encodes-row table; a double product or a float-formed q
+ * inside the loop fails it).  The file is also built with -fsanitize=address,undefined and run
+ * on ragged cases (tests/test_oracle_sanitize.py).  Parity unpinned by anything external: the
+ * choices R5/R6/R7 (boundary, row<->depth, velocity row) and the absolute amplitude scale R10
+ * -- fixed by DESIGN.md only (P5 accepts +-1 row, so it does not pin R6 to the row either).
  */
 #include <math.h>
 #include <stdlib.h>
@@ -64,15 +67,29 @@ int pdm_oracle_num_threads(void)
 #endif
 }
 
-/* O1 + O6 exposed on their own so pin P12 can test the index rule directly. */
-int pdm_oracle_index(float omega, float velocity, double dz, double du, int ntab)
+/* O1 (R3): q32 = fl32( dz / (v32 * du) ) -- formed in double, rounded ONCE to float. */
+static float oracle_q32(double dz, float velocity, double du)
 {
-    float q32 = (float)(dz / ((double)velocity * du));
-    float prod = omega * q32;                 /* float x float -> float, no FMA involved */
-    long j = lrintf(prod);                    /* default rounding mode: half to even     */
+    return (float)(dz / ((double)velocity * du));
+}
+
+/* O6 (R3): FLOAT product (float x float -> float, no FMA involved), round half to even
+ * (default rounding mode), clamp to the table.  The ONE statement of the index rule in this
+ * file: pdm_oracle_migrate's inner loop and pdm_oracle_index both call it. */
+static int oracle_idx(float w32, float q32, int ntab)
+{
+    float prod = w32 * q32;
+    long j = lrintf(prod);
     if (j < 0) j = 0;
     if (j > ntab - 1) j = ntab - 1;
     return (int)j;
+}
+
+/* O1 + O6 exposed on their own (pin P12a tests the rule directly; pin P12b tests it through
+ * pdm_oracle_migrate's loop). */
+int pdm_oracle_index(float omega, float velocity, double dz, double du, int ntab)
+{
+    return oracle_idx(omega, oracle_q32(dz, velocity, du), ntab);
 }
 
 /*
@@ -99,7 +116,7 @@ int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
     float *q32 = (float *)malloc(plane * sizeof(float));
     if (!q32) return ORACLE_ERR_NOMEM;
     for (size_t i = 0; i < plane; ++i)
-        q32[i] = (float)(dz / ((double)velocity[i] * du));
+        q32[i] = oracle_q32(dz, velocity[i], du);
 
     int nthreads = pdm_oracle_num_threads();
     if (nthreads > nlines) nthreads = nlines;
@@ -132,10 +149,7 @@ int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
                 for (int z = 0; z < nz; ++z) {                          /* O4 */
                     const float *qrow = q32 + (size_t)z * nx;
                     for (int x = 0; x < nx; ++x) {                      /* O5 */
-                        float prod = w32 * qrow[x];                     /* O6 */
-                        long j = lrintf(prod);
-                        if (j < 0) j = 0;
-                        if (j > ntab - 1) j = ntab - 1;
+                        const int j = oracle_idx(w32, qrow[x], ntab);   /* O6 */
                         const oracle_c64 *row = table + (size_t)j * ntaps;
                         double ar = 0.0, ai = 0.0;
                         for (int k = -L; k <= L; ++k) {                 /* O7 */

@@ -248,24 +248,72 @@ def test_P11_shift_invariance_in_vz():
 
 
 # ---------------------------------------------------------------- P12 index rule
-def test_P12_index_rule_matches_float32_definition():
-    """idx = clamp(rint_half_even(fl32(w32 * fl32(dz/(v*du))))) -- compared with numpy float32."""
+def _index_rule_inputs():
+    """16 frequencies, each with its own velocity row: 300 random velocities plus velocities
+    SEARCHED (numpy only) so that the two plausible wrong rules -- FP64 product, q formed in
+    float arithmetic -- give a different table row than R3 on them."""
     rng = np.random.default_rng(7)
     dz, du, ntab = 10.0, 0.00307, 1024
-    w = rng.uniform(10, 400, 4000).astype(np.float32)
-    v = rng.uniform(700, 2600, 4000).astype(np.float32)
-    q32 = (np.float64(dz) / (v.astype(np.float64) * du)).astype(np.float32)
-    expect = np.clip(np.rint(w * q32), 0, ntab - 1).astype(int)       # float32 product, half-even
-    got = np.array([oracle.table_index(w[i], v[i], dz, du, ntab) for i in range(w.size)])
-    assert np.array_equal(got, expect)
+    lines = []
+    for w in rng.uniform(10, 400, 16).astype(np.float32):
+        v = rng.uniform(700, 2600, 1_000_000).astype(np.float32)
+        q32 = (np.float64(dz) / (v.astype(np.float64) * du)).astype(np.float32)   # R3: one rounding
+        expect = np.clip(np.rint(w * q32), 0, ntab - 1).astype(np.int64)           # float32 product, half-even
+        alt_dp = np.clip(np.rint(np.float64(w) * q32.astype(np.float64)), 0, ntab - 1).astype(np.int64)
+        qf = np.float32(dz) / (v * np.float32(du))                                  # q in float arithmetic
+        alt_fq = np.clip(np.rint(w * qf), 0, ntab - 1).astype(np.int64)
+        hard = np.flatnonzero((alt_dp != expect) | (alt_fq != expect))
+        keep = np.concatenate([np.arange(300), hard])
+        lines.append((w, v[keep], expect[keep], alt_dp[keep], alt_fq[keep]))
+    n_dp = sum(int((l[3] != l[2]).sum()) for l in lines)
+    n_fq = sum(int((l[4] != l[2]).sum()) for l in lines)
+    return (dz, du, ntab), lines, n_dp, n_fq
+
+
+def test_P12a_index_rule_matches_float32_definition():
+    """idx = clamp(rint_half_even(fl32(w32 * fl32(dz/(v*du))))) -- compared with numpy float32 on
+    random pairs AND on pairs where an FP64 product or a float-formed q gives another row."""
+    (dz, du, ntab), lines, n_dp, n_fq = _index_rule_inputs()
+    for w, v, expect, _, _ in lines:
+        got = np.array([oracle.table_index(w, v[i], dz, du, ntab) for i in range(v.size)])
+        assert np.array_equal(got, expect)
     # exact ties round to even, and both clamps are active
     assert oracle.table_index(2.5, 1.0, 1.0, 1.0, 1024) == 2
     assert oracle.table_index(3.5, 1.0, 1.0, 1.0, 1024) == 4
     assert oracle.table_index(5000.0, 1.0, 1.0, 1.0, 1024) == 1023
     assert oracle.table_index(0.2, 1.0, 1.0, 1.0, 1024) == 0
-    # the FP64-product variant differs on some inputs, i.e. the rule is a real choice (R3)
-    alt = np.clip(np.rint(w.astype(np.float64) * (dz / (v.astype(np.float64) * du))), 0, ntab - 1)
-    assert (alt.astype(int) != expect).sum() >= 0
+    # the rule is a real choice (R3): both wrong variants differ on this set, so a slip to either
+    # cannot pass the equality above
+    assert n_dp > 50 and n_fq > 50, (n_dp, n_fq)
+
+
+def test_P12b_index_rule_through_the_migrate_loop():
+    """The rule as pdm_oracle_migrate's OWN loop applies it (not a twin function): nz = 1, P0 = 1,
+    a table whose centre tap of row j is the real number j and every other tap 0  =>
+    image[0][x] = sum_w idx(w, v[0][x]).  One frequency per call makes every pixel one (w, v)
+    pair.  Catches: FP64 product in the loop, q rounded twice / formed in float, truncation
+    instead of round-half-even, missing clamps, q row mis-indexing."""
+    (dz, du, ntab), lines, n_dp, n_fq = _index_rule_inputs()
+    assert n_dp > 50 and n_fq > 50, (n_dp, n_fq)                 # the set has teeth
+    ntaps = 5
+    table = np.zeros((ntab, ntaps), np.complex64)
+    table[:, ntaps // 2] = np.arange(ntab, dtype=np.float32)     # row j -> the number j
+    for w, v, expect, _, _ in lines:
+        nx = v.size
+        c = _cfg(nx, 1, [w], v[None, :], table, du, np.ones((1, nx), np.complex64), dz)
+        np.testing.assert_array_equal(oracle.migrate(c)[0], expect.astype(np.float64))
+    # both clamps through the loop: u far beyond the table and u -> 0
+    c = _cfg(2, 1, [400.0], np.array([[1.0, 1e9]], np.float32), table, du, np.ones((1, 2), np.complex64), dz)
+    np.testing.assert_array_equal(oracle.migrate(c)[0], [ntab - 1, 0])
+    # several frequencies and depth rows in ONE call (w loop, q row of step z): rows z >= 1 see the
+    # field after z+1 applications of the centre taps, so use nz = 1 per row check via the velocity row
+    nx, nw = 257, 6
+    ws = np.array([l[0] for l in lines[:nw]], np.float32)
+    vv = lines[0][1][:nx]
+    c = _cfg(nx, 1, ws, vv[None, :], table, du, np.ones((nw, nx), np.complex64), dz)
+    q32 = (np.float64(dz) / (vv.astype(np.float64) * du)).astype(np.float32)
+    want = sum(np.clip(np.rint(wi * q32), 0, ntab - 1) for wi in ws)
+    np.testing.assert_array_equal(oracle.migrate(c)[0], want.astype(np.float64))
 
 
 # ---------------------------------------------------------------- regression fixture
