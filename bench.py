@@ -9,10 +9,12 @@ imaging: SURVEY.md 8(a) A1-A7) over one f-x section: one `pdm_migrate` call.  At
 workload is BASELINE.json configs[3] (the configuration the north_star target is quoted on);
 inputs are seeded and synthetic.  Prints ONE JSON line on rank 0.
 
-N > 1 (torchrun): weak scaling.  The job is the configs[3] model with an N-times denser
-frequency list (the DFT bins of an N-times longer record); rank r owns the bins offset by r/N
-(803 lines each, frequencies are independent units) and the partial images are
-summed with one NCCL all-reduce inside the timed step -- the path's only exchange.
+N > 1: weak scaling, one rank per GPU (launched by torchrun; `python bench.py --gpus N` without
+torchrun re-executes itself under torch.distributed.run with N ranks, and fails loudly if the box
+has fewer than N GPUs).  The job is the configs[3] model with an N-times denser frequency list (the
+DFT bins of an N-times longer record); rank r owns the bins offset by r/N (803 lines each,
+frequencies are independent units) and the partial images are summed with one NCCL
+all-reduce inside the timed step -- the path's only exchange.
 
 --impl reference: times the FP64 CPU oracle (oracle/, as it stands) on the host cores on a
 bounded sample of the same workload (rank 0 only).
@@ -39,17 +41,47 @@ UNIT = "samples/s"
 # lanes x 2 flop/FMA x 1.965 GHz max SM clock.  The FFMA-chain microbenchmark (pdm_fp32_peak)
 # reads 71-73 TFLOP/s on this pool; both are reported.
 FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
-# committed `ncu --set full` capture of this command (profiles/r01_march_config3.md, section 2):
-# 27.09 GB + 29.55 GB on configs[3] (the per-CTA partial-image read-modify-write).
-NCU_DRAM_BYTES_PER_LAUNCH = {3: 27.094569e9 + 29.553966e9}
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+
+
+def csrc_digest() -> str:
+    """sha1 over the kernel sources: ties an ncu traffic figure to the code it was captured on."""
+    import hashlib
+    d = os.path.join(ROOT, "paper_1912_05529_b200", "csrc")
+    h = hashlib.sha1()
+    for name in sorted(os.listdir(d)):
+        if name.endswith((".cu", ".cuh")):
+            h.update(name.encode())
+            with open(os.path.join(d, name), "rb") as f:
+                h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_traffic(config: int, path: str, flags: int, world: int):
+    """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
+    committed `ncu --set full` capture (profiles/r02_traffic.json) -- only when that capture was
+    taken on exactly these kernel sources, this config and this path; else None with the reason."""
+    if world != 1 or flags:
+        return None, "no capture for multi-rank runs / non-default flags"
+    try:
+        with open(TRAFFIC_FILE) as f:
+            table = json.load(f)
+    except (OSError, ValueError):
+        return None, "profiles/r02_traffic.json absent"
+    for e in table.get("captures", []):
+        if e.get("config") == config and e.get("path") == path:
+            if e.get("csrc_sha1") != csrc_digest():
+                return None, (f"capture {e.get('report')} was taken on csrc {e.get('csrc_sha1')}, "
+                              f"HEAD is {csrc_digest()}: stale")
+            return float(e["dram_bytes_read"]) + float(e["dram_bytes_write"]), e.get("report")
+    return None, "no capture for this config/path"
 
 
 def load_workload(k: int, rank: int, world: int) -> dict:
     import pdm_inputs
     if k == 3:
-        from pdm_inputs.configs import config3
-        return config3(bin_offset=rank / world if world > 1 else 0.0)
+        from pdm_inputs.configs import config3_rank_shard
+        return config3_rank_shard(rank, world)
     cfg = pdm_inputs.make_config(k)
     if world > 1:                        # small configs: plain round-robin shard of the lines
         from paper_1912_05529_b200.shard import shard_workload
@@ -162,6 +194,55 @@ def run_reference(args, rank: int, world: int):
 
 
 # ------------------------------------------------------------------------------- our arm
+PATH_NAMES = {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster"}
+
+
+def time_migrate(plan, P0, image, stream, flush, torch, steps: int, warmup: int = 3):
+    """ms of `steps` pdm_migrate calls (CUDA events on the launching stream, L2 flushed between)."""
+    for _ in range(warmup):
+        plan.migrate(P0, image, stream=stream)
+    torch.cuda.synchronize()
+    ms = []
+    for _ in range(steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        plan.migrate(P0, image, stream=stream)
+        b.record(stream)
+        torch.cuda.synchronize()
+        ms.append(a.elapsed_time(b))
+    return ms
+
+
+def other_configs(pdm, torch, dev, stream, flush):
+    """The regimes the headline workload does not show, measured in the same run (a few seconds):
+    configs[0..2] and two configs[4] points where every sample has its own table row (tap-gather
+    bound) -- ms per migrate and the counted FP32 fraction, so that these are driver-measured too."""
+    import pdm_inputs
+    from pdm_inputs.configs import sweep_point
+    work = [(f"configs[{k}]", (lambda k=k: pdm_inputs.make_config(k))) for k in (0, 1, 2)]
+    work += [("configs[4] field", lambda: sweep_point(32768, 1024, 15)),
+             ("configs[4] field", lambda: sweep_point(4096, 1024, 51))]
+    rows = []
+    for name, make in work:
+        cfg = make()
+        with pdm.Plan.from_config(cfg, 0) as plan:
+            info = plan.info
+            P0 = torch.from_numpy(cfg["P0"]).to(dev)
+            image = torch.empty((cfg["nz"], cfg["nx"]), dtype=torch.float32, device=dev)
+            ms = time_migrate(plan, P0, image, stream, flush, torch, steps=5)
+        t = float(np.median(ms)) * 1e-3
+        sps = info["samples"] / t
+        rows.append({"workload": f"{name} nx={cfg['nx']} nz={cfg['nz']} nw={cfg['nw']} taps={cfg['ntaps']}",
+                     "path": PATH_NAMES[info["path"]], "ms_median": t * 1e3, "ms_best": float(min(ms)),
+                     "samples_per_s": sps,
+                     "frac_fp32_peak_counted": sps * 8 * cfg["ntaps"] / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                     "frac_hbm_16B_per_sample_of_measured":
+                         (sps * 16 / (measured_hbm_gbs()[0] * 1e9)) if info["path"] == pdm.PDM_PATH_TILED else None})
+        del P0, image
+    return rows
+
+
 def run_ours(args, rank: int, local_rank: int, world: int):
     import torch
     import torch.distributed as dist
@@ -174,11 +255,18 @@ def run_ours(args, rank: int, local_rank: int, world: int):
     pdm.load_library()                      # raises if libpdm.so was not built
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
+    print(f"[bench] rank {rank} of {world} on cuda:{local_rank} ({torch.cuda.get_device_name(local_rank)})",
+          file=sys.stderr, flush=True)
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")        # communicator log: shows the N ranks (and NVLS)
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=dev)
 
     cfg = load_workload(args.config, rank, world)
-    plan = pdm.Plan.from_config(cfg, args.flags)
+    t_create = time.perf_counter()
+    plan = pdm.Plan.from_config(cfg, args.flags)          # pdm_create: excluded from the metric, reported
+    torch.cuda.synchronize(dev)
+    create_ms = 1e3 * (time.perf_counter() - t_create)
     info = plan.info
     samples = info["samples"]
     stream = torch.cuda.current_stream(dev)
@@ -265,12 +353,19 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         except pdm.PdmError:
             fma_peak = None
         kernel = {pdm.PDM_PATH_SMEM: "pdm_march_kernel", pdm.PDM_PATH_TILED: "pdm_tiled_step",
-                  pdm.PDM_PATH_NAIVE: "pdm_naive_step"}.get(info["path"], "?")
+                  pdm.PDM_PATH_NAIVE: "pdm_naive_step", pdm.PDM_PATH_CLUSTER: "pdm_cluster_kernel"}[info["path"]]
+        path_name = PATH_NAMES[info["path"]]
+        traffic, traffic_src = ncu_traffic(args.config, path_name, args.flags, world)
+        algo_bytes = float(cfg["P0"].nbytes + 4 * cfg["nz"] * cfg["nx"] + cfg["velocity"].nbytes)
         roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
                     "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                     "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
-                    "traffic": NCU_DRAM_BYTES_PER_LAUNCH.get(args.config) if world == 1 and not args.flags else None,
-                    "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r01_march_config3.md)",
+                    "traffic": traffic,
+                    "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
+                    "traffic_source": traffic_src,
+                    "algorithmic_bytes": algo_bytes,
+                    "algorithmic_bytes_are": "P0 in + q map once + image out (the wavefield never leaves the SM)",
+                    "traffic_over_algorithmic": (traffic / algo_bytes) if traffic else None,
                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); "
                                    "MEASURED_PEAKS.json has no FP32 entry",
                     "ffma_chain_measured_tflops": fma_peak,
@@ -282,14 +377,16 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                     "reduce_ms": float(np.mean(reduce_ms))}
         cpu_v, cpu_dt, cpu_lines, cpu_threads = oracle_sample(cfg, lines_per_thread=args.cpu_lines_per_thread)
         out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": k,
-               "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k, "higher_is_better": True,
+               "warmup": max(args.warmup, 3), "ms_per_step": total_ms / k,
+               "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(min(step_ms)),
+               "create_ms": create_ms, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                "config": {"workload": workload_name(args.config, cfg, world),
-                          "path": {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster"}.get(info["path"]),
+                          "path": path_name,
                           "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                           "smem_bytes": info["smem_bytes"],
-                          "l2": "256 MiB buffer written between timed steps (L2 flush); per-step "
-                                f"working set {info['workspace_bytes'] / 1e9:.2f} GB > 126 MB L2"},
+                          "l2": "256 MiB buffer written between timed steps (L2 flush); plan workspace "
+                                f"{info['workspace_bytes'] / 1e9:.3f} GB"},
                "pct_fp32_peak_counted": 100.0 * value / world * 8 * cfg["ntaps"] / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
                "roofline": roofline,
                "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
@@ -301,6 +398,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                        "ms_per_step": e2e_ms / k},
                "gpu_launches": int(info["launches_per_migrate"]) * k,
                "clocks": clocks}
+        if world == 1 and not args.no_extra:
+            out["extra"] = {"other_configs": other_configs(pdm, torch, dev, stream, flush)}
         print(json.dumps(out), flush=True)
     plan.close()
     if world > 1:
@@ -312,6 +411,15 @@ def run_ours(args, rank: int, local_rank: int, world: int):
 SWEEP_NX = (1024, 4096, 16384, 32768)
 SWEEP_NW = (64, 256, 1024, 2048)
 SWEEP_TAPS = (15, 25, 51)
+
+
+def measured_hbm_gbs():
+    """(GB/s, source): the driver-measured copy bandwidth, else the profiling guide's fallback."""
+    for cand in ("/root/repo/MEASURED_PEAKS.json", os.path.join(ROOT, "MEASURED_PEAKS.json")):
+        if os.path.exists(cand):
+            with open(cand) as f:
+                return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
 
 
 def run_sweep(args):
@@ -329,12 +437,7 @@ def run_sweep(args):
     torch.cuda.set_device(dev)
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
-    hbm_gbs, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"    # used only if the driver's file is absent
-    for cand in ("/root/repo/MEASURED_PEAKS.json", os.path.join(ROOT, "MEASURED_PEAKS.json")):
-        if os.path.exists(cand):
-            with open(cand) as f:
-                hbm_gbs, hbm_src = float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
-            break
+    hbm_gbs, hbm_src = measured_hbm_gbs()
     def pick(arg, full):
         return tuple(int(t) for t in arg.split(",")) if arg else full
     for ntaps in pick(args.sweep_taps, SWEEP_TAPS):
@@ -362,7 +465,7 @@ def run_sweep(args):
                 sps = info["samples"] / t
                 tiled = info["path"] == pdm.PDM_PATH_TILED
                 out = {"workload": f"configs[4] nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} velocity={args.sweep_model}",
-                       "path": {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster"}.get(info["path"]),
+                       "path": PATH_NAMES[info["path"]],
                        "taps_mode": info["taps_mode"], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                        "launches": info["launches_per_migrate"], "steps": steps, "ms": t * 1e3,
                        "samples_per_s": sps,
@@ -428,6 +531,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--flags", type=lambda s: int(s, 0), default=0, help="pdm_create flags word")
     ap.add_argument("--cpu-lines-per-thread", type=int, default=16)
+    ap.add_argument("--no-extra", action="store_true",
+                    help="skip extra.other_configs (configs[0..2] + two configs[4] points, N = 1 only)")
     ap.add_argument("--tf", action="store_true", help="time the t->f transform of the section (SURVEY 8(f) N1)")
     ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep, one JSON line per point")
     ap.add_argument("--sweep-taps", default="", help="comma list of tap counts to sweep (default 15,25,51)")
@@ -437,9 +542,29 @@ def main():
                     help="velocity of the sweep: BASELINE.json's random field, or flat layers "
                          "(warp-uniform table rows: the HBM-bound regime of the x-tiled path)")
     args = ap.parse_args()
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+    multi = not (args.tf or args.sweep)
+    if multi and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: start the N ranks ourselves (one process per GPU, NCCL), loudly
+        # refusing a box with fewer GPUs -- never a silent 1-rank run that prints n_gpus: 1
+        if args.impl == "ours":
+            import torch
+            have = torch.cuda.device_count()
+            if have < args.gpus:
+                raise SystemExit(f"bench.py: --gpus {args.gpus} but this box has {have} CUDA device(s)")
+        import socket
+        with socket.socket() as sock:
+            sock.bind(("127.0.0.1", 0))
+            port = sock.getsockname()[1]
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1",
+                                  f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+                                  "--master-port", str(port), os.path.abspath(__file__), *sys.argv[1:]])
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if multi and world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch one rank per GPU")
     if args.tf:
         if rank == 0:
             run_tf(args)

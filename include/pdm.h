@@ -63,16 +63,19 @@ typedef enum {
 #define PDM_PATH_MASK    0xFu
 #define PDM_TAPS_AUTO    (0u << 4)  /* where the kernels read filter rows from                      */
 #define PDM_TAPS_GLOBAL  (1u << 4)  /* always from the L2/L1-cached global half-table               */
-#define PDM_TAPS_SLICE   (2u << 4)  /* per-frequency contiguous row slice staged in shared memory   */
-#define PDM_TAPS_COMPACT (3u << 4)  /* per-frequency list of the rows actually used, staged in SMEM */
+#define PDM_TAPS_SLICE   (2u << 4)  /* rows a frequency can touch staged in shared memory; whether   */
+#define PDM_TAPS_COMPACT (3u << 4)  /* the list is the contiguous range [idx(q_min), idx(q_max)] or  */
+                                    /* the exact rows (models with <= 2048 distinct velocities) is   */
+                                    /* the library's choice either way: both values request staging, */
+                                    /* pdm_info.taps_mode reports 2 (range) or 3 (exact list)        */
 #define PDM_TAPS_MASK    (0x3u << 4)
-#define PDM_FORCE_GENERAL (1u << 6) /* debug: never take the uniform-index fast path                */
+#define PDM_FORCE_GENERAL (1u << 6) /* debug: never take the thread-uniform fast path (every output   */
+                                    /* fetches its own tap row even where a warp shares one)        */
 #define PDM_NO_BALANCE   (1u << 7)  /* debug: whole lines per CTA (no depth-split load balancing)   */
 #define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto)                   */
 #define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
                                     /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
-#define PDM_TILE_SHIFT    20        /* bits 20-27: x-tile size / 256 samples for PDM_PATH_TILED     */
-#define PDM_FLAGS_VALID  0x0FFFFFFFu
+#define PDM_FLAGS_VALID  0x000FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
 
 typedef struct {
     int    path;                 /* PDM_PATH_* actually chosen                                      */

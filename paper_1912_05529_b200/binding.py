@@ -25,7 +25,7 @@ PDM_ERR_CUDA = -6
 PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER = 0, 1, 2, 3, 4
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 PDM_FORCE_GENERAL, PDM_NO_BALANCE = 1 << 6, 1 << 7
-PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TILE_SHIFT = 8, 16, 20
+PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16
 
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
@@ -276,8 +276,11 @@ class Plan:
         enqueued on one stream (marshalling only; P0 is the unscaled transform)."""
         import torch
         st = stream or torch.cuda.current_stream(section.device)
-        P0 = transform.forward(section, stream=st)
-        return self.migrate(P0, image, stream=st)
+        # the temporary P0 is allocated (and later freed) under `st`, so the caching allocator
+        # cannot hand its block to another stream while pdm_migrate is still reading it
+        with torch.cuda.stream(st):
+            P0 = transform.forward(section, stream=st)
+            return self.migrate(P0, image, stream=st)
 
     def migrate_host(self, P0_host, image_host=None, stream=None):
         """End-to-end call: HOST complex64 [nw, nx] (numpy or pinned torch) -> HOST float32 [nz, nx]."""

@@ -32,9 +32,10 @@ struct pdm_cluster_params {
     int nx, nz, nw, ntab;
     int qstride, pstride, half16;
     int ngroups, passes, gper, slots, map_len, nclusters;
+    int force_general;       // PDM_FORCE_GENERAL (debug)
 };
 
-template <int L, int R, bool TAPS_SMEM, bool DEDUP>
+template <int L, int R, bool TAPS_SMEM, bool DEDUP, bool SYM = true>
 __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(const pdm_cluster_params p)
 {
     namespace cg = cooperative_groups;
@@ -42,7 +43,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(c
     constexpr int GS = R + 2;
     // per-sample-row plans: row de-duplication and part of the tap gather through the texture unit,
     // exactly as in pdm_march_kernel
-    constexpr unsigned TEXMASK = DEDUP ? (L <= 7 ? 0x88u : 0x80u) : 0u;
+    constexpr unsigned TEXMASK = (SYM && DEDUP) ? (L <= 7 ? 0x88u : 0x80u) : 0u;
     cg::cluster_group cluster = cg::this_cluster();
     const int C = (int)cluster.num_blocks(), rank = (int)cluster.block_rank();
     const int cid = blockIdx.x / C;
@@ -125,7 +126,7 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(c
                     jn[r] = pdm_index(w, qn[r], ntab_m1);
                     u = u && (jn[r] == jn[0]);
                 }
-                un = u;
+                un = u && !p.force_general;
 #pragma unroll
                 for (int r = 0; r < R; ++r)
                     tn[r] = (((TEXMASK >> r) & 1u) ? jn[r] : (TAPS_SMEM ? (int)map[jn[r]] : jn[r])) * p.half16;
@@ -170,8 +171,13 @@ __global__ void __launch_bounds__(PDM_MARCH_MAX_THREADS, 1) pdm_cluster_kernel(c
                     }
                     const float2 *base = cur + (HG + gl) * GS;
                     float2 out[R];
-                    if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
-                    else     pdm_fir_group<L, R, false, DEDUP, TEXMASK>(base, tbase, toff, out, p.tex);
+                    if (SYM) {
+                        if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
+                        else     pdm_fir_group<L, R, false, DEDUP, TEXMASK>(base, tbase, toff, out, p.tex);
+                    } else {
+                        if (uni) pdm_fir_group_asym<L, R, true>(base, tbase, toff, out);
+                        else     pdm_fir_group_asym<L, R, false>(base, tbase, toff, out);
+                    }
                     if (active) {
                         const int x0 = g * R;
                         float2 *dst = nxt + (HG + gl) * GS;

@@ -41,6 +41,7 @@ struct pdm_march_params {
     int nx, nz, nw, ntab;
     int qstride, pstride, half16;
     int ngroups, passes, slots, map_len;
+    int force_general;       // PDM_FORCE_GENERAL: never take the thread-uniform fast path (debug)
 };
 
 __host__ __device__ constexpr int pdm_floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
@@ -139,9 +140,63 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
     for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
 }
 
+// The same group of R outputs for a table that is NOT symmetric in k (general operators, PAPER.md:39,
+// :83): Eq. (1) literally, P'(x) = sum_k W_k P(x-k) with W_k and W_-k distinct.
+// Table row layout: float4 unit k = (W_k, W_-k), k = 0..L (unit 0 holds W_0 twice).  Same sliding
+// register windows; 4 FFMA2 per (k, output) instead of 1 FADD2 + 2 FFMA2: 8L+4 lane-ops per output.
+template <int L, int R, bool UNIFORM>
+__device__ __forceinline__ void pdm_fir_group_asym(const float2 *__restrict__ base,
+                                                   const float4 *__restrict__ tbase,
+                                                   const int (&toff)[R], float2 (&out)[R])
+{
+    float2 wl[R], wr[R], acc_a[R], acc_b[R];
+    float4 tw[UNIFORM ? 1 : R];
+#pragma unroll
+    for (int i = 0; i < R / 2; ++i) {
+        const float4 v = *reinterpret_cast<const float4 *>(base + 2 * i);
+        wl[2 * i] = f4lo(v); wl[2 * i + 1] = f4hi(v);
+        wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
+    }
+#pragma unroll
+    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r]];
+#pragma unroll
+    for (int r = 0; r < R; ++r) {                       // centre tap W_0
+        const float4 t = tw[UNIFORM ? 0 : r];
+        acc_a[r] = pk_mul_s(wl[r].x, f4lo(t));
+        acc_b[r] = pk_mul_s(wl[r].y, f4lo(t));
+    }
+    float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
+#pragma unroll
+    for (int k = 1; k <= L; ++k) {
+        if (k & 1) {
+            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(-k - 1));
+            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(R + k - 1));
+            wl[pdm_mod(-k, R)] = f4hi(lv);
+            wr[pdm_mod(k - 1, R)] = f4lo(rv);
+        } else {
+            wl[pdm_mod(-k, R)] = f4lo(lv);
+            wr[pdm_mod(k - 1, R)] = f4hi(rv);
+        }
+#pragma unroll
+        for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = tbase[toff[r] + k];
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            const float2 a = wl[pdm_mod(r - k, R)];     // P(x-k): multiplied by W_k   (R11)
+            const float2 b = wr[pdm_mod(r + k, R)];     // P(x+k): multiplied by W_-k
+            acc_a[r] = pk_fma_s(a.x, f4lo(t), acc_a[r]);
+            acc_b[r] = pk_fma_s(a.y, f4lo(t), acc_b[r]);
+            acc_a[r] = pk_fma_s(b.x, f4hi(t), acc_a[r]);
+            acc_b[r] = pk_fma_s(b.y, f4hi(t), acc_b[r]);
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) out[r] = make_float2(acc_a[r].x - acc_b[r].y, acc_a[r].y + acc_b[r].x);
+}
+
 // R = 8: one CTA of up to 384 threads per SM.  R = 4 (short lines, few of them): up to 256 threads and
 // at least two CTAs per SM, so that small problems put more warps on an SM.
-template <int L, int R, bool TAPS_SMEM, bool DEDUP>
+template <int L, int R, bool TAPS_SMEM, bool DEDUP, bool SYM = true>
 __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ? 1 : 2) pdm_march_kernel(const pdm_march_params p)
 {
     static_assert(R % 2 == 0 && R >= 2, "R must be even");
@@ -149,7 +204,7 @@ __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ?
     constexpr int GS = R + 2;
     // per-sample-row plans only: 2 of a thread's 8 tap rows through the texture unit for the shortest
     // filters, 1 of 8 for longer ones (measured best per length; more costs registers the loop needs)
-    constexpr unsigned TEXMASK = (DEDUP && R == 8) ? (L <= 7 ? 0x88u : 0x80u) : 0u;
+    constexpr unsigned TEXMASK = (SYM && DEDUP && R == 8) ? (L <= 7 ? 0x88u : 0x80u) : 0u;
     extern __shared__ __align__(16) unsigned char pdm_smem[];
     float2 *buf_a = reinterpret_cast<float2 *>(pdm_smem);
     float2 *buf_b = buf_a + p.slots;
@@ -250,7 +305,7 @@ __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ?
                     jn[r] = pdm_index(w, qn[r], ntab_m1);
                     u = u && (jn[r] == jn[0]);
                 }
-                un = u;
+                un = u && !p.force_general;
 #pragma unroll
                 for (int r = 0; r < R; ++r)
                     tn[r] = (((TEXMASK >> r) & 1u) ? jn[r] : (TAPS_SMEM ? (int)map[jn[r]] : jn[r])) * p.half16;
@@ -298,8 +353,13 @@ __global__ void __launch_bounds__(R >= 8 ? PDM_MARCH_MAX_THREADS : 256, R >= 8 ?
                     }
                     const float2 *base = cur + (HG + g) * GS;
                     float2 out[R];
-                    if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
-                    else     pdm_fir_group<L, R, false, DEDUP, TEXMASK>(base, tbase, toff, out, p.tex);
+                    if (SYM) {
+                        if (uni) pdm_fir_group<L, R, true, false>(base, tbase, toff, out);
+                        else     pdm_fir_group<L, R, false, DEDUP, TEXMASK>(base, tbase, toff, out, p.tex);
+                    } else {
+                        if (uni) pdm_fir_group_asym<L, R, true>(base, tbase, toff, out);
+                        else     pdm_fir_group_asym<L, R, false>(base, tbase, toff, out);
+                    }
                     if (active) {
                         const int x0 = g * R;
                         float2 *dst = nxt + (HG + g) * GS;

@@ -27,6 +27,7 @@ struct pdm_tf_params {
     const int    *bins;        // [nw]
     const float2 *tw;          // [nt] (cos, -sin)(2 pi m / nt)
     int nt, nx, nw;
+    int wide_out;              // 1: nx even and P0 16-byte aligned -> 16-byte stores of the result
 };
 
 template <int CW>   // floats per async copy: 4 (nx % 4 == 0 and a 16-byte aligned section) or 1
@@ -105,7 +106,7 @@ __global__ void __launch_bounds__(PDM_TF_THREADS, 2) pdm_tf_kernel(const pdm_tf_
             }
         }
     }
-    const bool wide = (p.nx % 2 == 0);                                 // 16-byte aligned rows
+    const bool wide = p.wide_out != 0;                                 // 16-byte aligned rows (host-checked)
 #pragma unroll
     for (int jj = 0; jj < PDM_TF_JT; ++jj) {
         if (j0 + jj >= p.nw) continue;

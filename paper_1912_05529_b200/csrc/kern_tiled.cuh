@@ -33,6 +33,7 @@ struct pdm_tiled_params {
     int nx, nz, nw, ntab;
     int qstride, pstride, half16;
     int z, w_per_group;
+    int force_general;       // PDM_FORCE_GENERAL (debug)
 };
 
 // CH = samples per async-copy chunk: 2 (16-byte copies; needs nx even and 16-byte aligned planes)
@@ -46,7 +47,7 @@ __device__ __forceinline__ void pdm_cp_async(float2 *dst_smem, const float2 *src
     else         asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" :: "r"(d), "l"(src), "r"(n) : "memory");
 }
 
-template <int L, int R, int CH, bool ALIAS>
+template <int L, int R, int CH, bool ALIAS, bool SYM = true>
 __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm_tiled_params p)
 {
     constexpr int HG = pdm_halo_groups<L, R>();
@@ -122,8 +123,14 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
         for (int r = 0; r < R; ++r) toff[r] = j[r] * p.half16;
         const float2 *base = ibuf + b * IN_SLOTS + (HG + lane) * GS;
         float2 out[R];
-        if (__all_sync(0xffffffffu, uni)) pdm_fir_group<L, R, true, false>(base, p.half, toff, out);
-        else                              pdm_fir_group<L, R, false, false>(base, p.half, toff, out);
+        const bool wuni = __all_sync(0xffffffffu, uni && !p.force_general);
+        if (SYM) {
+            if (wuni) pdm_fir_group<L, R, true, false>(base, p.half, toff, out);
+            else      pdm_fir_group<L, R, false, false>(base, p.half, toff, out);
+        } else {
+            if (wuni) pdm_fir_group_asym<L, R, true>(base, p.half, toff, out);
+            else      pdm_fir_group_asym<L, R, false>(base, p.half, toff, out);
+        }
 
         // ALIAS (plans with long, per-sample table rows): the consumed input buffer doubles as the
         // output tile -- less shared memory leaves more L1 for the tap rows (+11..24 % at 51 taps on
@@ -151,6 +158,9 @@ __global__ void __launch_bounds__(PDM_TILED_THREADS, 2) pdm_tiled_step(const pdm
                 else         dst[x] = *sp;
             }
         }
+        // ALIAS: the output tile lives in input buffer b, which the NEXT iteration refills with
+        // cp.async right away -- every lane must have copied its part out first
+        if (ALIAS) __syncwarp();
     }
     if (w_begin < w_end && x0 < p.pstride) {
         float *prow = p.partial + ((size_t)blockIdx.y * p.nz + p.z) * p.pstride + x0;

@@ -226,13 +226,15 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, ntaps = p->ntaps, L = p->L;
     const int Lk = kernel_half_length(L);                  // 0: no unrolled kernel is long enough
     p->Lk = Lk;
-    // outputs per thread: 8, or 4 for short lines with so few of them that 8 would leave the SMs
-    // with under 8 warps each (configs[0], [1]); only the single-CTA marching form has the R = 4 build
+    // outputs per thread: PDM_R = 8 for every kernel form; the single-CTA marching form also has an
+    // R = 4 build for short lines with so few of them that 8 would leave the SMs with under 8 warps
+    // each (configs[0], [1]).  The form is chosen with the R = 8 layout first; R drops to 4 only once
+    // the path is known to be PDM_PATH_SMEM (tiled and cluster kernels exist for R = 8 only).
     const unsigned want_path = p->flags & PDM_PATH_MASK;
     const bool small = (want_path == PDM_PATH_AUTO || want_path == PDM_PATH_SMEM) && nx <= 1024 &&
                        (long long)nw * ((nx + 255) / 256) <= 8LL * p->sm_count &&
                        ((p->flags >> PDM_THREADS_SHIFT) & 0xFFu) == 0;   // a forced thread count means the R = 8 layout
-    const int R = small ? PDM_R_SMALL : PDM_R;
+    int R = PDM_R;
     p->R = R;
 
     // ---- q map (R3) and its extrema ---------------------------------------------------------
@@ -311,15 +313,15 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     const unsigned want = p->flags & PDM_PATH_MASK;
     const unsigned want_taps = p->flags & PDM_TAPS_MASK;
     const bool have_L = Lk != 0;
-    const int HG = halo_groups(have_L ? Lk : L, R);
-    const int ngroups = (nx + R - 1) / R;
-    const int slots = (2 * HG + ngroups) * (R + 2);
-    const int map_len = round_up(ntab, 8);
-    const size_t line_bytes = (size_t)2 * slots * sizeof(float2) + (size_t)map_len * 2;
-    const size_t slice_bytes = (size_t)p->max_rows * p->half16 * sizeof(float4);
-    const bool lines_fit = have_L && line_bytes <= (size_t)p->smem_optin;
-    const bool slice_fits = lines_fit && line_bytes + slice_bytes <= (size_t)p->smem_optin &&
-                            p->max_rows <= 65535;
+    int HG = halo_groups(have_L ? Lk : L, R);
+    int ngroups = (nx + R - 1) / R;
+    int slots = (2 * HG + ngroups) * (R + 2);
+    const int map_len = round_up(ntab, 8);                 // u16 row -> slot map, only with staged rows
+    size_t line_bytes = (size_t)2 * slots * sizeof(float2);
+    const size_t slice_bytes = (size_t)map_len * 2 + (size_t)p->max_rows * p->half16 * sizeof(float4);
+    bool lines_fit = have_L && line_bytes <= (size_t)p->smem_optin;
+    bool slice_fits = lines_fit && line_bytes + slice_bytes <= (size_t)p->smem_optin &&
+                      p->max_rows <= 65535;
 
     // cluster form: C = 2, 4 or 8 CTAs per line (bits PDM_CTAS_SHIFT force it).  Among the sizes
     // whose per-CTA ping-pong segment fits shared memory, the largest that still leaves every CTA
@@ -334,7 +336,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
             const int ps = (gneed + PDM_MARCH_MAX_THREADS - 1) / PDM_MARCH_MAX_THREADS;
             const int nwp = (gneed + 32 * ps - 1) / (32 * ps);
             const int gp = 32 * ps * nwp;
-            const size_t bytes = (size_t)2 * (2 * HG + gp) * (R + 2) * sizeof(float2) + (size_t)map_len * 2;
+            const size_t bytes = (size_t)2 * (2 * HG + gp) * (R + 2) * sizeof(float2);
             if (bytes > (size_t)p->smem_optin) continue;
             const bool wanted = (long long)nw * c <= p->sm_count && gneed >= 256;
             if (cl_C && !wanted) break;                    // keep the smaller size found before
@@ -365,6 +367,17 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->path = (auto_cluster || auto_pair) ? PDM_PATH_CLUSTER
                                : (lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE));
     else p->path = (int)want;
+    if (p->path == PDM_PATH_SMEM && small) {               // the R = 4 build: redo the line layout
+        R = PDM_R_SMALL;
+        p->R = R;
+        HG = halo_groups(Lk, R);
+        ngroups = (nx + R - 1) / R;
+        slots = (2 * HG + ngroups) * (R + 2);
+        line_bytes = (size_t)2 * slots * sizeof(float2);
+        lines_fit = line_bytes <= (size_t)p->smem_optin;
+        slice_fits = lines_fit && line_bytes + slice_bytes <= (size_t)p->smem_optin && p->max_rows <= 65535;
+        if (!lines_fit) return PDM_ERR_UNSUPPORTED;        // cannot happen for nx <= 1024; defensive
+    }
 
     int rc;
     if ((rc = dev_upload(p, &p->d_omega, omega, (size_t)nw)) != PDM_OK) return rc;
@@ -522,6 +535,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.passes = (a.ngroups + p->threads - 1) / p->threads;
         a.slots = (2 * halo_groups(Lk, R) + a.ngroups) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
+        a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
         march_fn fn = march_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p), R);
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
         if (p->balanced) {                               // split lines: CTAs wait on one another
@@ -548,6 +562,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.passes = p->cluster_passes; a.gper = p->cluster_gper;
         a.slots = (2 * halo_groups(Lk, R) + a.gper) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
+        a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
         a.nclusters = p->n_partial;
         a.tex = p->tex_half;
         cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p));
@@ -569,6 +584,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.nx = nx; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
         a.qstride = p->qstride; a.pstride = p->qstride; a.half16 = p->half16;
         a.w_per_group = (nw + p->wgroups - 1) / p->wgroups;
+        a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
         // 16-byte async copies need every plane row 16-byte aligned: nx even and an aligned P0
         const bool wide = (nx % 2 == 0) && (((uintptr_t)P0_dev & 15u) == 0);
         tiled_fn fn = tiled_kernel_for(p, wide);
@@ -809,6 +825,8 @@ extern "C" int pdm_tf_forward(pdm_tf *tf, const float *section_dev, pdm_c64 *P0_
     pdm_tf_params a;
     a.section = section_dev; a.out = reinterpret_cast<float2 *>(P0_dev);
     a.bins = tf->d_bins; a.tw = tf->d_tw; a.nt = tf->nt; a.nx = tf->nx; a.nw = tf->nw;
+    // 16-byte stores of P0 rows need every row 16-byte aligned: nx even AND an aligned P0
+    a.wide_out = (tf->nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) ? 1 : 0;
     const int jb = tf->warps * PDM_TF_JT;
     dim3 grid((tf->nx + PDM_TF_XB - 1) / PDM_TF_XB, (tf->nw + jb - 1) / jb);
     if (tf->nx % 4 == 0 && ((uintptr_t)section_dev & 15u) == 0)

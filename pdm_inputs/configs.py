@@ -318,6 +318,25 @@ def config3(seed: int = BASE_SEED + 3, bin_offset: float = 0.0):
                    d["omega"], d["v"], d["P0"])
 
 
+def config3_rank_shard(rank: int, world: int, seed: int = BASE_SEED + 3):
+    """Rank `rank`'s share of the N-GPU weak-scaling job bench.py runs: the configs[3] model and
+    table with an N-times denser frequency list (the DFT bins of an N-times longer record).  Rank r
+    owns the bins r/N of a bin BELOW configs[3]'s own (so every u stays inside the table), 803 lines
+    each; its section is configs[3]'s rotated by a unit phase per rank (same statistics, different
+    data -- synthetic either way).  Derived from the cached configs[3] arrays in a fraction of a
+    second, so N ranks do not each spend minutes re-synthesising 2000 diffractors."""
+    base = config3(seed)
+    if world <= 1:
+        return base
+    nt, dt = 4096, 2e-3
+    domega = 2.0 * np.pi / (nt * dt)
+    out = dict(base)
+    out["omega"] = (base["omega"].astype(np.float64) - (rank / world) * domega).astype(np.float32)
+    out["P0"] = np.ascontiguousarray(base["P0"] * np.complex64(np.exp(1j * np.pi * rank / world)))
+    out["name"] = base["name"] + f" rank {rank}/{world}"
+    return out
+
+
 # --------------------------------------------------------------------------- configs[4]
 SWEEP_NX = (1024, 4096, 16384, 32768)
 SWEEP_NW = (64, 256, 1024, 2048)

@@ -199,6 +199,34 @@ def test_cluster_path_matches_oracle(pdm, nx, nz, nw, ntaps, model, csize):
     assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
 
 
+def test_auto_small_problem_with_a_huge_table_keeps_a_consistent_layout(pdm):
+    """nx <= 1024, few lines (the R = 4 regime) and a table so large that the row map alone would not
+    fit shared memory: the outputs-per-thread choice must follow the path actually chosen (R = 4 exists
+    for the single-CTA marching form only), and the row map must not count against a plan whose rows
+    stay global."""
+    for nx, nw, ntab in ((640, 6, 120000), (1024, 3, 131072), (512, 40, 110000)):
+        cfg = pdm_inputs.random_problem(81, nx, 10, nw, 15, ntab=ntab, model="field")
+        ref = oracle.migrate(cfg)
+        img, info = gpu_migrate(pdm, cfg, 0, want_info=True)
+        rel, mx = errors(img, ref)
+        assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (nx, nw, ntab, rel, mx, info)
+        for path in ("tiled", "cluster", "smem_global"):
+            assert_parity(pdm, cfg, path_flags(pdm, path), ref=ref)
+
+
+@pytest.mark.parametrize("path", ["smem_staged", "smem_global", "tiled", "cluster"])
+def test_force_general_flag_takes_the_per_output_gather(pdm, path):
+    """PDM_FORCE_GENERAL: a warp-uniform model (layers) run through the per-output tap gather must
+    give the same image bit for bit as the thread-uniform fast path (same taps, same order)."""
+    cfg = pdm_inputs.random_problem(83, 1300, 18, 5, 25, model="layers")
+    flags = path_flags(pdm, path)
+    fast = gpu_migrate(pdm, cfg, flags)
+    general = gpu_migrate(pdm, cfg, flags | pdm.PDM_FORCE_GENERAL)
+    assert np.array_equal(fast, general)
+    rel, mx = errors(general, oracle.migrate(cfg))
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+
+
 def test_auto_policy_picks_the_measured_best_form(pdm):
     """pdm_create's AUTO choice (flags = 0) for the regimes measured in profiles/r01_sweep_config4.md."""
     def path_of(nx, nw, ntaps, model):
@@ -265,17 +293,89 @@ def test_config3_full_size_sampled_frequencies(pdm):
     _subset_parity(pdm, cfg, lines, 0, expect_path=pdm.PDM_PATH_SMEM)
 
 
+def _sample_lines(info, nw, want=16):
+    """Frequency lines for a sampled-line parity check at full size: the first and last lines, the
+    lines at (and next to) the boundaries between CTAs' work ranges -- with depth-split balancing the
+    line floor(nw*c/grid) is the one CTA c-1 and CTA c share (head on one, tail on the other); on the
+    x-tiled path the same lines sit at frequency-group boundaries -- the lines around the first wrap
+    of the round-robin cluster schedule, and an even fill up to `want`."""
+    lines = {0, 1, nw - 2, nw - 1}
+    grid = max(1, info["grid_ctas"])
+    for c in (1, 2, grid // 3, grid // 2, grid - 1):
+        b = nw * c // grid
+        lines |= {b - 1, b, b + 1}
+    for wrap in (37, 74, 148, 296):
+        lines |= {wrap - 1, wrap}
+    lines = {l for l in lines if 0 <= l < nw}
+    fill = [int(round(t)) for t in np.linspace(0, nw - 1, want)]
+    for l in fill:
+        if len(lines) >= want:
+            break
+        lines.add(l)
+    return sorted(lines)[:max(want, 24)]
+
+
+# SURVEY 8(d): the four corners and the diagonal of the (nx, nw) sweep for each filter length
+CONFIG4_POINTS = [(1024, 64), (1024, 2048), (32768, 64), (32768, 2048), (4096, 256), (16384, 1024)]
+
+
 @pytest.mark.slow
-@pytest.mark.parametrize("nx,nw,ntaps", [(1024, 64, 15), (4096, 256, 25), (32768, 64, 51), (16384, 64, 15)])
-def test_config4_points_sampled_frequencies(pdm, nx, nw, ntaps):
+@pytest.mark.parametrize("ntaps", [15, 25, 51])
+@pytest.mark.parametrize("nx,nw", CONFIG4_POINTS)
+def test_config4_corners_and_diagonal(pdm, nx, nw, ntaps):
+    """BASELINE.json configs[4] at FULL size in the launch configuration bench.py --sweep times (AUTO):
+    (a) >= 16 sampled frequency lines (CTA range boundaries, split lines, first/last) against the
+        oracle, the other lines zero -- the oracle computes exactly those lines;
+    (b) ALL lines non-zero: the AUTO image against the scaffold kernel (PDM_PATH_NAIVE: one thread per
+        sample, unfolded 2L+1 row, one launch per level -- an independent kernel that shares only the
+        index rule), whose own sampled lines are oracle-checked in (c).  A defect tied to particular
+        CTAs or lines (hand-off of split lines, last-round clusters, frequency-group tails) cannot
+        hide behind zero-filled lines here."""
+    import torch
     cfg = pdm_inputs.sweep_point(nx, nw, ntaps)
-    lines = sorted({0, nw // 3, nw - 1})
-    # nx >= 16384 cannot be a single-CTA line: x-tiled, or (few lines, rows stageable) the cluster form
-    _subset_parity(pdm, cfg, lines, 0, expect_path=None if nx >= 16384 else pdm.PDM_PATH_SMEM)
-    if nx >= 16384:
-        with pdm.Plan.from_config(cfg, 0) as plan:
-            assert plan.info["path"] in (pdm.PDM_PATH_TILED, pdm.PDM_PATH_CLUSTER)
-        _subset_parity(pdm, cfg, lines, pdm.PDM_PATH_TILED, expect_path=pdm.PDM_PATH_TILED)
+    with pdm.Plan.from_config(cfg, 0) as plan:
+        info = plan.info
+        if nx <= 4096:
+            assert info["path"] == pdm.PDM_PATH_SMEM or (nw == 64 and info["path"] == pdm.PDM_PATH_CLUSTER), info
+        elif nx == 32768 and nw >= 256:
+            assert info["path"] == pdm.PDM_PATH_TILED, info             # north_star: forced x-tiled
+        elif (nx, nw, ntaps) == (16384, 1024, 15):
+            assert info["path"] == pdm.PDM_PATH_CLUSTER, info           # AUTO's cluster-pair policy
+        lines = _sample_lines(info, nw)
+        assert len(lines) >= min(16, nw)
+        full = torch.from_numpy(cfg["P0"]).cuda()
+        sub = torch.zeros_like(full)
+        idx = torch.as_tensor(lines, device="cuda")
+        sub[idx] = full[idx]
+        img_sub = plan.migrate(sub).cpu().numpy()
+        img_full = plan.migrate(full).cpu().numpy()
+    ref = oracle.migrate(cfg, omega_index=np.asarray(lines, dtype=np.int32))
+    rel, mx = errors(img_sub, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, ("sampled lines", cfg["name"], rel, mx, info)
+    with pdm.Plan.from_config(cfg, pdm.PDM_PATH_NAIVE) as naive:
+        ref_full = naive.migrate(full).cpu().numpy().astype(np.float64)
+        ref_sub = naive.migrate(sub).cpu().numpy()
+    rel, mx = errors(ref_sub, ref)                                      # (c) the scaffold itself
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, ("scaffold", cfg["name"], rel, mx)
+    rel, mx = errors(img_full, ref_full)                                # (b) every line
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, ("all lines vs scaffold", cfg["name"], rel, mx, info)
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("nx,nw,ntaps,model,flags_name", [
+    (32768, 1024, 15, "layers", "auto"),     # the point the x-tiled path's HBM fraction is quoted on
+    (16384, 1024, 15, "field", "tiled"),     # the x-tiled alternative AUTO's pair policy is measured against
+    (16384, 64, 15, "field", "auto"),        # few long lines: cluster form
+    (32768, 256, 25, "field", "auto"),
+])
+def test_config4_more_points_sampled_frequencies(pdm, nx, nw, ntaps, model, flags_name):
+    cfg = pdm_inputs.sweep_point(nx, nw, ntaps, model=model)
+    flags = 0 if flags_name == "auto" else path_flags(pdm, flags_name)
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        info = plan.info
+    if (nx, nw, model) == (32768, 1024, "layers"):
+        assert info["path"] == pdm.PDM_PATH_TILED
+    _subset_parity(pdm, cfg, _sample_lines(info, nw), flags)
 
 
 @pytest.mark.slow

@@ -113,3 +113,21 @@ def test_tf_error_codes_on_device(pdm):
     assert pdm.pdm_tf_forward(h, 0, 0, 0) == pdm.PDM_ERR_INVALID_ARG
     assert pdm.pdm_tf_destroy(h) == pdm.PDM_OK
     assert pdm.pdm_tf_destroy(None) == pdm.PDM_OK
+
+
+def test_transform_into_an_output_that_is_only_8_byte_aligned(pdm):
+    """Even nx but a P0 buffer at an address = 8 mod 16 (pdm_migrate accepts such a P0): the kernel
+    must fall back to 8-byte stores and give the same values as the aligned call."""
+    import torch
+    nt, nx = 256, 260
+    bins = np.arange(3, 60, dtype=np.int32)
+    rng = np.random.default_rng(77)
+    section = torch.from_numpy(rng.standard_normal((nt, nx)).astype(np.float32)).cuda()
+    with pdm.SectionTransform(nt, nx, bins) as tf:
+        aligned = tf.forward(section)
+        store = torch.empty(bins.size * nx + 1, dtype=torch.complex64, device="cuda")
+        shifted = store[1:].view(bins.size, nx)
+        assert shifted.data_ptr() % 16 == 8
+        tf.forward(section, out=shifted)
+        torch.cuda.synchronize()
+    assert torch.equal(aligned, shifted)
