@@ -35,9 +35,10 @@ typedef enum {
     PDM_ERR_INVALID_ARG = -1,      /* NULL pointer, dim <= 0, ntaps even or < 1, tab_du <= 0,
                                       non-finite or <= 0 velocity / omega, unknown flag bits       */
     PDM_ERR_TABLE_RANGE = -2,      /* some rint(w*q) > ntab-1 (kernels still clamp defensively)    */
-    PDM_ERR_TABLE_ASYMMETRIC = -3, /* table[j][L+k] != table[j][L-k] bitwise: the kernels fold the
-                                      symmetric taps (W_k == W_-k, north_star) and would silently
-                                      compute something else                                       */
+    PDM_ERR_TABLE_ASYMMETRIC = -3, /* only with PDM_REQUIRE_SYMMETRIC: table[j][L+k] != table[j][L-k]
+                                      bitwise.  Without that flag such a table selects the general
+                                      kernels (full 2L+1 row, 8L+4 lane-ops per sample instead of
+                                      6L+4) and pdm_info.table_symmetric reports 0                 */
     PDM_ERR_UNSUPPORTED = -4,      /* not a CC 10.x device; forced path impossible for this nx;
                                       ntaps above PDM_MAX_TAPS; a forced SMEM / TILED / CLUSTER path
                                       with more than 51 taps (the longest unrolled kernel; shorter
@@ -72,10 +73,12 @@ typedef enum {
 #define PDM_FORCE_GENERAL (1u << 6) /* debug: never take the thread-uniform fast path (every output   */
                                     /* fetches its own tap row even where a warp shares one)        */
 #define PDM_NO_BALANCE   (1u << 7)  /* debug: whole lines per CTA (no depth-split load balancing)   */
+#define PDM_REQUIRE_SYMMETRIC (1u << 20) /* refuse a table that is not bitwise symmetric in k        */
+                                    /* (PDM_ERR_TABLE_ASYMMETRIC) instead of taking the general kernels */
 #define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto)                   */
 #define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
                                     /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
-#define PDM_FLAGS_VALID  0x000FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
+#define PDM_FLAGS_VALID  0x001FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
 
 typedef struct {
     int    path;                 /* PDM_PATH_* actually chosen                                      */
@@ -88,6 +91,7 @@ typedef struct {
     int    launches_per_migrate; /* kernels one pdm_migrate call enqueues                           */
     int    sm_count;
     int    last_cuda_error;      /* cudaError_t of the last failing CUDA call (0 if none)           */
+    int    table_symmetric;      /* 1: W_k == W_-k bitwise, folded kernels; 0: general kernels      */
     double samples;              /* nx*nz*nw: extrapolated (z,w,x) points per migrate               */
     double counted_flops;        /* 8*(2L+1)*samples (metric definition, BASELINE.json north_star)  */
     double executed_lane_ops;    /* (6L+4)*samples FP32 lane operations with symmetric folding      */
@@ -102,8 +106,9 @@ typedef struct {
  *   omega     HOST  float[nw], rad/s, any order, finite, > 0.
  *   velocity  HOST  float[nz][nx], m/s, finite, > 0: the MIGRATION velocity; the library computes
  *             exactly u = w*dz/velocity (the caller passes v/2 for two-way-time data, R2).
- *   table     HOST  pdm_c64[ntab][ntaps]; table[j][L+k] = W_k(u_j), u_j = j*tab_du, k = -L..L (R11);
- *             must be bitwise symmetric in k.
+ *   table     HOST  pdm_c64[ntab][ntaps]; table[j][L+k] = W_k(u_j), u_j = j*tab_du, k = -L..L, and
+ *             W_k multiplies P(x-k) (Eq. (1), R11).  A table that is bitwise symmetric in k runs
+ *             on the folded kernels; any other table on the general ones.
  *   flags     PDM_PATH_* | PDM_TAPS_* | tuning bits.
  * The caller may free all its arrays on return.  The plan is bound to the CUDA device that is
  * current at the call.  Not thread-safe per plan; different plans are independent.

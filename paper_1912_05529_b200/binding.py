@@ -24,7 +24,7 @@ PDM_ERR_CUDA = -6
 
 PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER = 0, 1, 2, 3, 4
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
-PDM_FORCE_GENERAL, PDM_NO_BALANCE = 1 << 6, 1 << 7
+PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC = 1 << 6, 1 << 7, 1 << 20
 PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16
 
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
@@ -40,7 +40,7 @@ class PdmInfo(ctypes.Structure):
                 ("grid_ctas", ctypes.c_int), ("threads_per_cta", ctypes.c_int),
                 ("ctas_per_sm", ctypes.c_int), ("smem_bytes", ctypes.c_int),
                 ("launches_per_migrate", ctypes.c_int), ("sm_count", ctypes.c_int),
-                ("last_cuda_error", ctypes.c_int),
+                ("last_cuda_error", ctypes.c_int), ("table_symmetric", ctypes.c_int),
                 ("samples", ctypes.c_double), ("counted_flops", ctypes.c_double),
                 ("executed_lane_ops", ctypes.c_double), ("workspace_bytes", ctypes.c_double)]
 

@@ -19,6 +19,9 @@ UNITS = [("pdm_api.cu", [], "pdm_api.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=0"], "tu_march0.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=1"], "tu_march1.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=2"], "tu_march2.o"),
+         ("tu_asym.cu", ["-DPDM_TU_PART=0"], "tu_asym0.o"),
+         ("tu_asym.cu", ["-DPDM_TU_PART=1"], "tu_asym1.o"),
+         ("tu_asym.cu", ["-DPDM_TU_PART=2"], "tu_asym2.o"),
          ("tu_cluster.cu", [], "tu_cluster.o"),
          ("tu_tiled.cu", [], "tu_tiled.o")]
 HEADERS = ["pdm_common.cuh", "pdm_dispatch.cuh", "kern_naive.cuh", "kern_peak.cuh", "kern_march.cuh",

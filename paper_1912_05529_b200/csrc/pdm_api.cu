@@ -108,11 +108,15 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
     for (size_t i = 0; i < plane; ++i)
         if (!(velocity[i] > 0.f) || !std::isfinite(velocity[i])) return PDM_ERR_INVALID_ARG;
     const int L = (ntaps - 1) / 2;
-    for (int j = 0; j < ntab; ++j) {
+    // W_k == W_-k bit for bit in every row: the folded kernels (north_star); otherwise the general
+    // kernels apply the full 2L+1 row (Eq. (1) literally, R11)
+    bool symmetric = true;
+    for (int j = 0; j < ntab && symmetric; ++j) {
         const pdm_c64 *row = table + (size_t)j * ntaps + L;
         for (int k = 1; k <= L; ++k)
-            if (memcmp(&row[k], &row[-k], sizeof(pdm_c64)) != 0) return PDM_ERR_TABLE_ASYMMETRIC;
+            if (memcmp(&row[k], &row[-k], sizeof(pdm_c64)) != 0) { symmetric = false; break; }
     }
+    if (!symmetric && (flags & PDM_REQUIRE_SYMMETRIC)) return PDM_ERR_TABLE_ASYMMETRIC;
 
     int dev = 0;
     cudaDeviceProp prop;
@@ -127,6 +131,7 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
     memset(p, 0, sizeof(*p));
     p->nx = nx; p->nz = nz; p->nw = nw; p->ntab = ntab; p->ntaps = ntaps; p->L = L;
     p->dx = dx; p->dz = dz; p->du = tab_du; p->flags = flags;
+    p->sym = symmetric ? 1 : 0;
     p->device = dev; p->sm_count = prop.multiProcessorCount;
     p->smem_optin = (int)prop.sharedMemPerBlockOptin;
 
@@ -139,17 +144,44 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
 // ------------------------------------------------------------------------------------------------
 // kernel dispatch: filter half-lengths with a fully unrolled, register-tiled instantiation
 // ------------------------------------------------------------------------------------------------
-static march_fn march_kernel_for(int L, bool taps_smem, bool dedup = false, int R = PDM_R)
+static march_fn march_kernel_for(const pdm_plan *p, bool taps_smem, bool dedup, int R)
 {
-    march_fn f = pdm_march_kernel_part0(L, taps_smem, dedup, R);
+    const int L = p->Lk;
+    march_fn f;
+    if (!p->sym) {
+        f = pdm_march_kernel_asym_part0(L, taps_smem);
+        if (!f) f = pdm_march_kernel_asym_part1(L, taps_smem);
+        if (!f) f = pdm_march_kernel_asym_part2(L, taps_smem);
+        return f;
+    }
+    f = pdm_march_kernel_part0(L, taps_smem, dedup, R);
     if (!f) f = pdm_march_kernel_part1(L, taps_smem, dedup, R);
     if (!f) f = pdm_march_kernel_part2(L, taps_smem, dedup, R);
     return f;
 }
-static cluster_fn cluster_kernel_for(int L, bool taps_smem, bool dedup) { return pdm_cluster_kernel_for(L, taps_smem, dedup); }
+static cluster_fn cluster_kernel_for(const pdm_plan *p, bool taps_smem, bool dedup)
+{
+    const int L = p->Lk;
+    if (!p->sym) {
+        cluster_fn f = pdm_cluster_kernel_asym_part0(L, taps_smem);
+        if (!f) f = pdm_cluster_kernel_asym_part1(L, taps_smem);
+        if (!f) f = pdm_cluster_kernel_asym_part2(L, taps_smem);
+        return f;
+    }
+    return pdm_cluster_kernel_for(L, taps_smem, dedup);
+}
 // output tile aliased onto the consumed input tile: only where it pays (long per-sample rows)
-static bool tiled_alias(const pdm_plan *p) { return p->contiguous_rows != 0 && p->Lk == 25; }
-static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide) { return pdm_tiled_kernel_for(p->Lk, wide, tiled_alias(p)); }
+static bool tiled_alias(const pdm_plan *p) { return p->sym && p->contiguous_rows != 0 && p->Lk == 25; }
+static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide)
+{
+    if (!p->sym) {
+        tiled_fn f = pdm_tiled_kernel_asym_part0(p->Lk, wide);
+        if (!f) f = pdm_tiled_kernel_asym_part1(p->Lk, wide);
+        if (!f) f = pdm_tiled_kernel_asym_part2(p->Lk, wide);
+        return f;
+    }
+    return pdm_tiled_kernel_for(p->Lk, wide, tiled_alias(p));
+}
 // Filter lengths without an instantiation of their own run on the next longer one with the extra
 // taps set to zero (x + 0*s == x exactly), so every odd length up to the longest instantiation
 // takes the unrolled kernels; 0 = longer than all of them (scaffold only).
@@ -202,7 +234,7 @@ static void build_segments(int nw, int nz, int grid, bool balance,
 // Row de-duplication inside a thread (pdm_fir_group DEDUP) pays where nearly every sample has its
 // own table row and the filter is short enough to leave registers: measured +4..7 % on the marching
 // path for taps <= 35 on random-field models, -4 % at 51 taps, -10 % on the 128-register tiled kernel.
-static bool use_dedup(const pdm_plan *p) { return p->contiguous_rows != 0 && p->Lk <= 17; }
+static bool use_dedup(const pdm_plan *p) { return p->sym && p->contiguous_rows != 0 && p->Lk <= 17; }
 
 // the half table as a linear float4 texture: the per-sample-row kernel variants fetch part of their
 // tap rows through the texture unit (a second gather path next to the LSU)
@@ -231,7 +263,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     // each (configs[0], [1]).  The form is chosen with the R = 8 layout first; R drops to 4 only once
     // the path is known to be PDM_PATH_SMEM (tiled and cluster kernels exist for R = 8 only).
     const unsigned want_path = p->flags & PDM_PATH_MASK;
-    const bool small = (want_path == PDM_PATH_AUTO || want_path == PDM_PATH_SMEM) && nx <= 1024 &&
+    const bool small = p->sym && (want_path == PDM_PATH_AUTO || want_path == PDM_PATH_SMEM) && nx <= 1024 &&
                        (long long)nw * ((nx + 255) / 256) <= 8LL * p->sm_count &&
                        ((p->flags >> PDM_THREADS_SHIFT) & 0xFFu) == 0;   // a forced thread count means the R = 8 layout
     int R = PDM_R;
@@ -259,13 +291,19 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     }
 
     // ---- half table: rows k = 0..L as float4 pairs (W_2t, W_2t+1), odd number of float4 per row
-    p->half16 = ((std::max(L, Lk) + 2) / 2) | 1;            // rows padded with zero taps up to Lk
+    // general (asymmetric) tables: unit k = (W_k, W_-k), k = 0..L, same odd padding
+    p->half16 = (p->sym ? (std::max(L, Lk) + 2) / 2 : std::max(L, Lk) + 1) | 1;   // rows padded with zero taps up to Lk
     std::vector<float4> half((size_t)ntab * p->half16, make_float4(0.f, 0.f, 0.f, 0.f));
     for (int j = 0; j < ntab; ++j)
         for (int k = 0; k <= L; ++k) {
             const pdm_c64 w = table[(size_t)j * ntaps + L + k];
-            float4 &d = half[(size_t)j * p->half16 + k / 2];
-            if (k & 1) { d.z = w.re; d.w = w.im; } else { d.x = w.re; d.y = w.im; }
+            if (p->sym) {
+                float4 &d = half[(size_t)j * p->half16 + k / 2];
+                if (k & 1) { d.z = w.re; d.w = w.im; } else { d.x = w.re; d.y = w.im; }
+            } else {
+                const pdm_c64 wm = table[(size_t)j * ntaps + L - k];
+                half[(size_t)j * p->half16 + k] = make_float4(w.re, w.im, wm.re, wm.im);
+            }
         }
 
     // ---- per-omega list of rows that omega can touch ---------------------------------------------
@@ -401,7 +439,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         }
         p->threads = threads;
         p->smem_bytes = (int)(line_bytes + (p->taps_in_smem ? slice_bytes : 0));
-        march_fn fn = march_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p), R);
+        march_fn fn = march_kernel_for(p, p->taps_in_smem != 0, use_dedup(p), R);
         PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          p->smem_bytes));
         int per_sm = 0;
@@ -446,7 +484,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         p->threads = 32 * nwarps;
         p->cluster_size = C; p->cluster_gper = gper; p->cluster_passes = passes;
         p->smem_bytes = (int)(seg_bytes + (p->taps_in_smem ? slice_bytes : 0));
-        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p));
+        cluster_fn fn = cluster_kernel_for(p, p->taps_in_smem != 0, use_dedup(p));
         PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          p->smem_bytes));
         int max_clusters = 0;
@@ -536,7 +574,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.slots = (2 * halo_groups(Lk, R) + a.ngroups) * (R + 2);
         a.map_len = round_up(p->ntab, 8);
         a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
-        march_fn fn = march_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p), R);
+        march_fn fn = march_kernel_for(p, p->taps_in_smem != 0, use_dedup(p), R);
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
         if (p->balanced) {                               // split lines: CTAs wait on one another
             // hand-off flags start empty even if an earlier migrate on this plan was cut short
@@ -565,7 +603,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
         a.nclusters = p->n_partial;
         a.tex = p->tex_half;
-        cluster_fn fn = cluster_kernel_for(Lk, p->taps_in_smem != 0, use_dedup(p));
+        cluster_fn fn = cluster_kernel_for(p, p->taps_in_smem != 0, use_dedup(p));
         cudaLaunchConfig_t cfg = {};
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
@@ -675,7 +713,8 @@ extern "C" int pdm_get_info(const pdm_plan *p, pdm_info *out)
     out->sm_count = p->sm_count; out->last_cuda_error = p->last_cuda_error;
     out->samples = (double)p->nx * (double)p->nz * (double)p->nw;
     out->counted_flops = 8.0 * p->ntaps * out->samples;
-    out->executed_lane_ops = (6.0 * (p->Lk ? p->Lk : p->L) + 4.0) * out->samples;   // zero-padded taps are executed too
+    out->executed_lane_ops = ((p->sym ? 6.0 : 8.0) * (p->Lk ? p->Lk : p->L) + 4.0) * out->samples;   // zero-padded taps are executed too
+    out->table_symmetric = p->sym;
     out->workspace_bytes = p->workspace_bytes;
     return PDM_OK;
 }

@@ -24,3 +24,15 @@ march_fn pdm_march_kernel_part1(int L, bool taps_smem, bool dedup, int R);
 march_fn pdm_march_kernel_part2(int L, bool taps_smem, bool dedup, int R);
 cluster_fn pdm_cluster_kernel_for(int L, bool taps_smem, bool dedup);
 tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias);
+
+// general (asymmetric-table) builds: R = PDM_R, no row de-duplication / texture share (tu_asym.cu,
+// compiled in the same three parts of the filter-length list)
+march_fn   pdm_march_kernel_asym_part0(int L, bool taps_smem);
+march_fn   pdm_march_kernel_asym_part1(int L, bool taps_smem);
+march_fn   pdm_march_kernel_asym_part2(int L, bool taps_smem);
+cluster_fn pdm_cluster_kernel_asym_part0(int L, bool taps_smem);
+cluster_fn pdm_cluster_kernel_asym_part1(int L, bool taps_smem);
+cluster_fn pdm_cluster_kernel_asym_part2(int L, bool taps_smem);
+tiled_fn   pdm_tiled_kernel_asym_part0(int L, bool wide);
+tiled_fn   pdm_tiled_kernel_asym_part1(int L, bool wide);
+tiled_fn   pdm_tiled_kernel_asym_part2(int L, bool wide);

@@ -390,11 +390,12 @@ def tiny_random_problem(seed: int, nx=9, nz=3, nw=2, L=2, ntab=7, symmetric=True
 
 
 def random_problem(seed: int, nx: int, nz: int, nw: int, ntaps: int, ntab: int = 256,
-                   model: str = "field", designed: bool = False):
+                   model: str = "field", designed: bool = False, symmetric: bool = True):
     """Mid-size seeded problem with a chosen velocity structure: 'const' | 'layers' | 'field' | 'white'.
 
     Table: random symmetric rows scaled so that sum_k |W_k| < 1 (stable for any index
-    pattern) unless `designed`, in which case the D1-D4 design is used.
+    pattern) unless `designed`, in which case the D1-D4 design is used; `symmetric=False` gives
+    W_-k independent of W_k (the general-operator kernels), same bound.
     """
     rng = np.random.default_rng([seed, nx, nz, nw, ntaps])
     dx = dz = 10.0
@@ -417,8 +418,14 @@ def random_problem(seed: int, nx: int, nz: int, nw: int, ntaps: int, ntab: int =
         table = filters.random_symmetric_table(rng, ntab, ntaps, scale=1.0)
         table = (table / (np.abs(table).sum(axis=1, keepdims=True) * 1.02)).astype(np.complex64)
         L = (ntaps - 1) // 2
-        for k in range(1, L + 1):
-            table[:, L - k] = table[:, L + k]
+        if symmetric:
+            for k in range(1, L + 1):
+                table[:, L - k] = table[:, L + k]
+        else:                                   # general operator: independent W_k and W_-k, same stability bound
+            rng_a = np.random.default_rng([seed, 77])
+            left = (rng_a.standard_normal((ntab, L)) + 1j * rng_a.standard_normal((ntab, L))).astype(np.complex64)
+            table[:, :L] = left * (np.abs(table[:, L + 1:]).sum(axis=1, keepdims=True) /
+                                   np.maximum(np.abs(left).sum(axis=1, keepdims=True), 1e-30)).astype(np.float32) * np.float32(0.98)
     P0 = np.empty((nw, nx), dtype=np.complex64)
     P0.real = rng.standard_normal((nw, nx), dtype=np.float32)
     P0.imag = rng.standard_normal((nw, nx), dtype=np.float32)

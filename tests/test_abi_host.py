@@ -75,14 +75,14 @@ def test_argument_validation_happens_before_any_device_use(lib):
         ((*args[:5], bad_omega, *args[6:]), pdm.PDM_ERR_INVALID_ARG),
         ((*args[:6], bad_v, *args[7:]), pdm.PDM_ERR_INVALID_ARG),
         ((*args[:7], even, args[8]), pdm.PDM_ERR_INVALID_ARG),
-        ((*args[:7], asym, args[8]), pdm.PDM_ERR_TABLE_ASYMMETRIC),
+        ((*args[:7], asym, args[8], pdm.PDM_REQUIRE_SYMMETRIC), pdm.PDM_ERR_TABLE_ASYMMETRIC),
         ((*args[:8], -1.0), pdm.PDM_ERR_INVALID_ARG),
         ((*args[:8], float("nan")), pdm.PDM_ERR_INVALID_ARG),
     ]
     for a, want in cases:
         rc, h = pdm.pdm_create(*a)
         assert rc == want and h is None
-    for bad_flags in (1 << 30, 1 << 20, 5, 15):            # unknown bits; undefined path numbers
+    for bad_flags in (1 << 30, 1 << 27, 5, 15):            # unknown bits; undefined path numbers
         rc, h = pdm.pdm_create(*args, flags=bad_flags)
         assert rc == pdm.PDM_ERR_INVALID_ARG and h is None, bad_flags
     # NULL handles

@@ -199,6 +199,31 @@ def test_cluster_path_matches_oracle(pdm, nx, nz, nw, ntaps, model, csize):
     assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
 
 
+@pytest.mark.parametrize("path", PATHS + ["auto"])
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps", [
+    ("field", 300, 20, 5, 15), ("white", 1000, 12, 4, 25), ("layers", 2500, 16, 5, 31),
+    ("const", 129, 30, 3, 35), ("field", 4100, 10, 3, 51), ("layers", 77, 9, 2, 3)])
+def test_asymmetric_tables_run_on_the_general_kernels(pdm, path, model, nx, nz, nw, ntaps):
+    """SURVEY 8(f) N3 (Eq. (1) literally): a table with W_k != W_-k is no longer
+    refused -- every kernel form has a general (unfolded) build.  The oracle applies the full row in
+    the x-k orientation (R11), so a transposed operand or a swapped W_k/W_-k fails here."""
+    cfg = pdm_inputs.random_problem(19, nx, nz, nw, ntaps, model=model, symmetric=False)
+    L = (ntaps - 1) // 2
+    assert not np.array_equal(cfg["table"][:, :L][:, ::-1], cfg["table"][:, L + 1:])
+    flags = 0 if path == "auto" else path_flags(pdm, path)
+    img, info = gpu_migrate(pdm, cfg, flags, want_info=True)
+    assert info["table_symmetric"] == 0
+    rel, mx = errors(img, oracle.migrate(cfg))
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (path, rel, mx, info)
+    # the symmetric twin of the same problem still reports the folded kernels
+    sym = pdm_inputs.random_problem(19, nx, nz, nw, ntaps, model=model)
+    with pdm.Plan.from_config(sym, flags) as plan:
+        assert plan.info["table_symmetric"] == 1
+    rc, h = pdm.pdm_create(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"],
+                           cfg["velocity"], cfg["table"], cfg["du"], flags | pdm.PDM_REQUIRE_SYMMETRIC)
+    assert rc == pdm.PDM_ERR_TABLE_ASYMMETRIC and h is None
+
+
 def test_auto_small_problem_with_a_huge_table_keeps_a_consistent_layout(pdm):
     """nx <= 1024, few lines (the R = 4 regime) and a table so large that the row map alone would not
     fit shared memory: the outputs-per-thread choice must follow the path actually chosen (R = 4 exists
