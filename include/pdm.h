@@ -204,6 +204,36 @@ int pdm_tf_create(pdm_tf **out, int nt, int nx, int nw, const int *bins);
 int pdm_tf_forward(pdm_tf *tf, const float *section_dev, pdm_c64 *P0_dev, void *cuda_stream);
 int pdm_tf_destroy(pdm_tf *tf);
 
+/*
+ * ---- extrapolator-table design on the device -------------------------------
+ * PAPER.md:39 (the filters trade length against maximum propagation angle), :83 ("Designing filters
+ * itself is optimization problem, it takes sometime ... we design the filters in advance and store
+ * it on the disk"), refs :163-165, :179-180.  The paper gives no recipe; pdm_design_table runs the
+ * projections-onto-convex-sets style iteration DESIGN.md states as D1-D4 for all ntab rows at once
+ * (one CTA per row, FP64): row j approximates the one-way phase shift of normalised wavenumber
+ * u_j = j*tab_du,
+ *     D(kappa) = exp(+i sqrt(u^2 - (r kappa)^2))  for |r kappa| <= u,  exp(-sqrt((r kappa)^2 - u^2)) beyond,
+ * kappa = k_x dx in [-pi, pi], r = dz/dx, with a 2L+1-tap symmetric filter that is exact (to the
+ * iteration's fixed point) on the passband |kappa| <= min((u/r) sin(angle), kappa_cap) and has
+ * |response| <= stop_cap elsewhere; the taps are finally divided by max(1, max|H|)(1+4e-7) so that
+ * the complex64 table is stable (|H| <= 1), and mirrored bit for bit (W_-k = W_k).
+ *   table_host  HOST pdm_c64[ntab][ntaps], overwritten; the layout pdm_create reads.
+ *   opts        HOST, NULL = the defaults in the comments below.
+ * Synchronous on cuda_stream (setup call: allocates and frees its own scratch).  Errors:
+ * PDM_ERR_INVALID_ARG, PDM_ERR_UNSUPPORTED (no CC 10.x device; L > 64; grid too large for shared
+ * memory), PDM_ERR_NOMEM, PDM_ERR_CUDA.
+ */
+typedef struct {
+    int    n_iter;               /* D2 iterations                      (default 200)                */
+    int    n_grid;               /* periodic kappa grid N, even        (default 2048)               */
+    int    n_check;              /* D3 kappa points on [0, pi]         (default 16384)              */
+    double passband_angle_deg;   /* maximum propagation angle          (default 55)                 */
+    double kappa_cap;            /* anti-alias cap of the passband     (default 0.8 pi)             */
+    double stop_cap;             /* |H| ceiling outside the passband   (default 0.9995)             */
+} pdm_design_opts;
+int pdm_design_table(pdm_c64 *table_host, int ntab, int ntaps, double tab_du, double dz_over_dx,
+                     const pdm_design_opts *opts, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

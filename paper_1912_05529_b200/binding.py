@@ -30,7 +30,7 @@ PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
                     "pdm_profile_enable", "pdm_profile_read",
-                    "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy")
+                    "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy", "pdm_design_table")
 
 
 class PdmInfo(ctypes.Structure):
@@ -46,6 +46,12 @@ class PdmInfo(ctypes.Structure):
 
     def as_dict(self) -> dict:
         return {name: getattr(self, name) for name, _ in self._fields_}
+
+
+class PdmDesignOpts(ctypes.Structure):
+    _fields_ = [("n_iter", ctypes.c_int), ("n_grid", ctypes.c_int), ("n_check", ctypes.c_int),
+                ("passband_angle_deg", ctypes.c_double), ("kappa_cap", ctypes.c_double),
+                ("stop_cap", ctypes.c_double)]
 
 
 class PdmError(RuntimeError):
@@ -91,6 +97,8 @@ def load_library(path: str | None = None):
     lib.pdm_tf_forward.argtypes = [vp, vp, vp, vp]
     lib.pdm_tf_destroy.restype = ci
     lib.pdm_tf_destroy.argtypes = [vp]
+    lib.pdm_design_table.restype = ci
+    lib.pdm_design_table.argtypes = [vp, ci, ci, cd, cd, ctypes.POINTER(PdmDesignOpts), vp]
     _lib = lib
     return lib
 
@@ -194,6 +202,22 @@ def pdm_tf_forward(handle, section_ptr: int, P0_ptr: int, cuda_stream: int = 0) 
 
 def pdm_tf_destroy(handle) -> int:
     return load_library().pdm_tf_destroy(handle)
+
+
+def pdm_design_table(ntab: int, ntaps: int, tab_du: float, dz_over_dx: float = 1.0, opts: dict | None = None,
+                     cuda_stream: int = 0) -> np.ndarray:
+    """-> complex64 [ntab, ntaps] designed on the device (D1-D4); `opts` overrides pdm_design_opts fields."""
+    out = np.empty((int(ntab), int(ntaps)), dtype=np.complex64)
+    o = None
+    if opts is not None:
+        o = PdmDesignOpts(200, 2048, 16384, 55.0, 0.8 * np.pi, 0.9995)
+        for k, v in opts.items():
+            setattr(o, k, v)
+    rc = load_library().pdm_design_table(out.ctypes.data, int(ntab), int(ntaps), float(tab_du), float(dz_over_dx),
+                                         ctypes.byref(o) if o is not None else None, ctypes.c_void_p(cuda_stream))
+    if rc != PDM_OK:
+        raise PdmError(rc, "pdm_design_table")
+    return out
 
 
 class SectionTransform:

@@ -16,6 +16,7 @@ LIB = os.path.join(_HERE, "libpdm.so")
 OBJDIR = os.path.join(_HERE, "build")
 # (source, extra defines, object name)
 UNITS = [("pdm_api.cu", [], "pdm_api.o"),
+         ("pdm_design.cu", [], "pdm_design.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=0"], "tu_march0.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=1"], "tu_march1.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=2"], "tu_march2.o"),
