@@ -194,7 +194,7 @@ def run_reference(args, rank: int, world: int):
 
 
 # ------------------------------------------------------------------------------- our arm
-PATH_NAMES = {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster"}
+PATH_NAMES = {1: "smem-marching", 2: "x-tiled", 3: "naive", 4: "cluster", 5: "packed"}
 
 
 def time_migrate(plan, P0, image, stream, flush, torch, steps: int, warmup: int = 3):
@@ -353,7 +353,8 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         except pdm.PdmError:
             fma_peak = None
         kernel = {pdm.PDM_PATH_SMEM: "pdm_march_kernel", pdm.PDM_PATH_TILED: "pdm_tiled_step",
-                  pdm.PDM_PATH_NAIVE: "pdm_naive_step", pdm.PDM_PATH_CLUSTER: "pdm_cluster_kernel"}[info["path"]]
+                  pdm.PDM_PATH_NAIVE: "pdm_naive_step", pdm.PDM_PATH_CLUSTER: "pdm_cluster_kernel",
+                  pdm.PDM_PATH_PACKED: "pdm_pack_kernel"}[info["path"]]
         path_name = PATH_NAMES[info["path"]]
         traffic, traffic_src = ncu_traffic(args.config, path_name, args.flags, world)
         algo_bytes = float(cfg["P0"].nbytes + 4 * cfg["nz"] * cfg["nx"] + cfg["velocity"].nbytes)

@@ -61,6 +61,10 @@ typedef enum {
                              /* the paper's own mapping, kept only as a cross-check    */
 #define PDM_PATH_CLUSTER 4u  /* main form with the line split over a thread-block cluster of 2, 4 or */
                              /* 8 CTAs, halos exchanged through distributed shared memory            */
+#define PDM_PATH_PACKED  5u  /* x-tiled AND temporally blocked (T depth steps per tile visit, planes   */
+                             /* cross HBM once per T steps, tiles moved by TMA) with 8 adjacent       */
+                             /* frequencies per quarter warp, which makes the per-sample tap gather   */
+                             /* bank-conflict free; any nx                        */
 #define PDM_PATH_MASK    0xFu
 #define PDM_TAPS_AUTO    (0u << 4)  /* where the kernels read filter rows from                      */
 #define PDM_TAPS_GLOBAL  (1u << 4)  /* always from the L2/L1-cached global half-table               */
@@ -78,6 +82,7 @@ typedef enum {
 #define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto)                   */
 #define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
                                     /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
+                                    /* with PDM_PATH_PACKED: depth steps per tile visit T (0 = auto) */
 #define PDM_FLAGS_VALID  0x001FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
 
 typedef struct {

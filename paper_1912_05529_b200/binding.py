@@ -22,7 +22,7 @@ PDM_ERR_UNSUPPORTED = -4
 PDM_ERR_NOMEM = -5
 PDM_ERR_CUDA = -6
 
-PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER = 0, 1, 2, 3, 4
+PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER, PDM_PATH_PACKED = 0, 1, 2, 3, 4, 5
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC = 1 << 6, 1 << 7, 1 << 20
 PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16

@@ -23,10 +23,13 @@ UNITS = [("pdm_api.cu", [], "pdm_api.o"),
          ("tu_asym.cu", ["-DPDM_TU_PART=0"], "tu_asym0.o"),
          ("tu_asym.cu", ["-DPDM_TU_PART=1"], "tu_asym1.o"),
          ("tu_asym.cu", ["-DPDM_TU_PART=2"], "tu_asym2.o"),
+         ("tu_pack.cu", ["-DPDM_TU_PART=0"], "tu_pack0.o"),
+         ("tu_pack.cu", ["-DPDM_TU_PART=1"], "tu_pack1.o"),
+         ("tu_pack.cu", ["-DPDM_TU_PART=2"], "tu_pack2.o"),
          ("tu_cluster.cu", [], "tu_cluster.o"),
          ("tu_tiled.cu", [], "tu_tiled.o")]
 HEADERS = ["pdm_common.cuh", "pdm_dispatch.cuh", "kern_naive.cuh", "kern_peak.cuh", "kern_march.cuh",
-           "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh", "kern_reduce.cuh"]
+           "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh", "kern_reduce.cuh", "kern_pack.cuh"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC"]
 

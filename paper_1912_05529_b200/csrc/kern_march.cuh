@@ -47,7 +47,8 @@ struct pdm_march_params {
 __host__ __device__ constexpr int pdm_floordiv(int a, int b) { return (a >= 0) ? a / b : -((-a + b - 1) / b); }
 __host__ __device__ constexpr int pdm_mod(int a, int b) { return a - pdm_floordiv(a, b) * b; }
 // slot offset (in float2) of sample x0+m relative to the slot of x0 (x0 = first sample of a group)
-template <int R> __host__ __device__ constexpr int pdm_soff(int m) { return m + 2 * pdm_floordiv(m, R); }
+// PAD = pad samples after every group of R (2 in the one-line-per-CTA layouts, 0 in the frequency-packed one)
+template <int R, int PAD = 2> __host__ __device__ constexpr int pdm_soff(int m) { return m + PAD * pdm_floordiv(m, R); }
 template <int L, int R> __host__ __device__ constexpr int pdm_halo_groups() { return (L + 1 + R - 1) / R; }
 
 __device__ __forceinline__ float2 f4lo(float4 v) { return make_float2(v.x, v.y); }
@@ -64,7 +65,7 @@ __device__ __forceinline__ float2 f4hi(float4 v) { return make_float2(v.z, v.w);
 // global half table; toff[r] is then a GLOBAL float4 index) through a 3-deep register ring, instead
 // of the LSU path: the texture unit is a second gather path whose bandwidth adds to the LSU's
 // (random 16-byte gathers, measured: shared memory 54 B/clk/SM, texture 23, mixed 3:1 71).
-template <int L, int R, bool UNIFORM, bool DEDUP, unsigned TEXMASK = 0u>
+template <int L, int R, bool UNIFORM, bool DEDUP, unsigned TEXMASK = 0u, int PAD = 2>
 __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
                                               const float4 *__restrict__ tbase,
                                               const int (&toff)[R], float2 (&out)[R],
@@ -109,8 +110,8 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
 #pragma unroll
     for (int k = 1; k <= L; ++k) {
         if (k & 1) {                                    // two new samples per side serve k and k+1
-            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(-k - 1));
-            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(R + k - 1));
+            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R, PAD>(-k - 1));
+            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R, PAD>(R + k - 1));
             wl[pdm_mod(-k, R)] = f4hi(lv);
             wr[pdm_mod(k - 1, R)] = f4lo(rv);
         } else {
@@ -144,7 +145,7 @@ __device__ __forceinline__ void pdm_fir_group(const float2 *__restrict__ base,
 // :83): Eq. (1) literally, P'(x) = sum_k W_k P(x-k) with W_k and W_-k distinct.
 // Table row layout: float4 unit k = (W_k, W_-k), k = 0..L (unit 0 holds W_0 twice).  Same sliding
 // register windows; 4 FFMA2 per (k, output) instead of 1 FADD2 + 2 FFMA2: 8L+4 lane-ops per output.
-template <int L, int R, bool UNIFORM>
+template <int L, int R, bool UNIFORM, int PAD = 2>
 __device__ __forceinline__ void pdm_fir_group_asym(const float2 *__restrict__ base,
                                                    const float4 *__restrict__ tbase,
                                                    const int (&toff)[R], float2 (&out)[R])
@@ -169,8 +170,8 @@ __device__ __forceinline__ void pdm_fir_group_asym(const float2 *__restrict__ ba
 #pragma unroll
     for (int k = 1; k <= L; ++k) {
         if (k & 1) {
-            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(-k - 1));
-            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(R + k - 1));
+            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R, PAD>(-k - 1));
+            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R, PAD>(R + k - 1));
             wl[pdm_mod(-k, R)] = f4hi(lv);
             wr[pdm_mod(k - 1, R)] = f4lo(rv);
         } else {

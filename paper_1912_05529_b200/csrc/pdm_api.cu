@@ -60,6 +60,7 @@ static void free_plan(pdm_plan *p)
     cudaFree(p->d_plane[0]); cudaFree(p->d_plane[1]); cudaFree(p->d_flags);
     cudaFree(p->d_handoff); cudaFree(p->d_segs); cudaFree(p->d_segoff);
     cudaFree(p->d_stage_p0); cudaFree(p->d_stage_img);
+    cudaFree(p->d_packrows); cudaFree(p->d_tile_ctas);
     for (int i = 0; i < 3; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
     delete p;
 }
@@ -99,7 +100,7 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
         return PDM_ERR_INVALID_ARG;
     if (flags & ~PDM_FLAGS_VALID) return PDM_ERR_INVALID_ARG;
     const unsigned path = flags & PDM_PATH_MASK;
-    if (path > PDM_PATH_CLUSTER) return PDM_ERR_INVALID_ARG;
+    if (path > PDM_PATH_PACKED) return PDM_ERR_INVALID_ARG;
     if (ntaps > PDM_MAX_TAPS) return PDM_ERR_UNSUPPORTED;
     if ((double)nz * (double)nx > 2.0e9 || (double)nw * (double)nx > 2.0e9) return PDM_ERR_UNSUPPORTED;
     for (int i = 0; i < nw; ++i)
@@ -181,6 +182,42 @@ static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide)
         return f;
     }
     return pdm_tiled_kernel_for(p->Lk, wide, tiled_alias(p));
+}
+static pack_fn pack_kernel_for(const pdm_plan *p)
+{
+    pack_fn f = pdm_pack_kernel_part0(p->Lk, p->sym != 0);
+    if (!f) f = pdm_pack_kernel_part1(p->Lk, p->sym != 0);
+    if (!f) f = pdm_pack_kernel_part2(p->Lk, p->sym != 0);
+    return f;
+}
+// TMA descriptor of a [nrows][row_samples] array of 8-byte samples (complex64 moved as opaque 64-bit
+// words), one-row boxes of `box` samples, out-of-range elements read as zero (R5).  The encoder is a
+// driver entry point resolved at run time: libpdm.so does not link libcuda (it must load without a GPU).
+typedef CUresult (*pdm_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+static int make_plane_map(pdm_plan *p, CUtensorMap *map, const void *base, int row_samples, int nrows, int box)
+{
+    static pdm_encode_fn enc = nullptr;
+    if (!enc) {
+        void *sym = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qr) != cudaSuccess ||
+            qr != cudaDriverEntryPointSuccess || !sym) {
+            cudaGetLastError();
+            return PDM_ERR_UNSUPPORTED;
+        }
+        enc = (pdm_encode_fn)sym;
+    }
+    const cuuint64_t dims[2] = { (cuuint64_t)row_samples, (cuuint64_t)nrows };
+    const cuuint64_t strides[1] = { (cuuint64_t)row_samples * sizeof(float2) };
+    const cuuint32_t boxd[2] = { (cuuint32_t)box, 1u }, estr[2] = { 1u, 1u };
+    const CUresult r = enc(map, CU_TENSOR_MAP_DATA_TYPE_UINT64, 2, const_cast<void *>(base), dims, strides, boxd, estr,
+                           CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                           CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) { p->last_cuda_error = (int)r; return PDM_ERR_CUDA; }
+    return PDM_OK;
 }
 // Filter lengths without an instantiation of their own run on the next longer one with the extra
 // taps set to zero (x + 0*s == x exactly), so every odd length up to the longest instantiation
@@ -401,6 +438,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     if (want == PDM_PATH_CLUSTER && !cl_C) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;  // (tiled_kernel_for has the same L list)
+    if (want == PDM_PATH_PACKED && !have_L) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_AUTO)
         p->path = (auto_cluster || auto_pair) ? PDM_PATH_CLUSTER
                                : (lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE));
@@ -536,6 +574,77 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)wgroups * nz * p->qstride)) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_plane[0], (size_t)nw * nx)) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_plane[1], (size_t)nw * nx)) != PDM_OK) return rc;
+    } else if (p->path == PDM_PATH_PACKED) {
+        // kern_pack.cuh: 8 adjacent frequencies per quarter warp, T depth steps per tile visit
+        p->taps_mode = 2;
+        const int NT = PDM_PACK_THREADS, W = PDM_PACK_W;
+        const unsigned tsel = (p->flags >> PDM_CTAS_SHIFT) & 0xFu;     // forced steps per visit
+        // default: the longest T whose recomputed halo stays under ~10 % of the tile
+        int T = tsel ? (int)tsel : (Lk <= 7 ? 4 : (Lk <= 12 ? 3 : 2));
+        T = std::min(T, nz);
+        const int passes = 1;
+        const int TXH = NT / W * R * passes;               // samples a CTA computes per line and step
+        const int H = round_up((T - 1) * Lk, R);           // recomputed halo per side
+        const int TX = TXH - 2 * H;
+        if (TX < 8 * R) return PDM_ERR_UNSUPPORTED;
+        p->nxp = round_up(nx, R);
+        const int w_load = TXH + 2 * R * HG + 2 * (W - 1); // samples per line incl. fetched halo and the per-line skew
+        const int nbox = (w_load + 255) / 256;
+        const int BW = round_up((w_load + nbox - 1) / nbox, 16);   // 128-byte aligned box starts
+        const int LS = nbox * BW;
+        const size_t lines_bytes = (size_t)PDM_PACK_NBUF * W * LS * sizeof(float2);
+        const size_t img_bytes = (size_t)T * TX * sizeof(float);
+        const int npacks = (nw + W - 1) / W;
+        std::vector<int2> packrows(npacks);
+        int maxrows = 0;
+        for (int k = 0; k < npacks; ++k) {
+            float wlo = INFINITY, whi = 0.f;
+            for (int i = k * W; i < std::min(nw, (k + 1) * W); ++i) { wlo = std::min(wlo, omega[i]); whi = std::max(whi, omega[i]); }
+            packrows[k] = make_int2(host_index(wlo, qmin, ntab), host_index(whi, qmax, ntab));
+            maxrows = std::max(maxrows, packrows[k].y - packrows[k].x + 1);
+        }
+        const size_t fixed = 128 + lines_bytes + img_bytes;
+        const size_t budget = (size_t)p->smem_optin - 1024;   // the kernel's static shared memory counts too
+        if (fixed >= budget) return PDM_ERR_UNSUPPORTED;
+        int cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
+        if (cap < maxrows) return PDM_ERR_UNSUPPORTED;     // one pack's rows must fit next to the line tiles
+        cap = std::min(cap, ntab);
+        p->pk_T = T; p->pk_TX = TX; p->pk_H = H; p->pk_LS = LS; p->pk_BW = BW; p->pk_nbox = nbox;
+        p->pk_cap = cap; p->pk_passes = passes; p->pk_npacks = npacks;
+        p->pk_ntiles = (nx + TX - 1) / TX;
+        p->threads = NT;
+        p->tile_x = TX;
+        p->smem_bytes = (int)(fixed + (size_t)cap * p->half16 * sizeof(float4));
+        pack_fn fn = pack_kernel_for(p);
+        if (!fn) return PDM_ERR_UNSUPPORTED;
+        PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+        const long long nitems = (long long)p->pk_ntiles * npacks;
+        if (nitems > 0x7fffffffLL) return PDM_ERR_UNSUPPORTED;
+        p->ctas_per_sm = 1;
+        p->grid = (int)std::min<long long>(nitems, p->sm_count);
+        const int nblocks = (nz + T - 1) / T;
+        p->launches = 2 * nblocks;
+        p->n_partial = p->grid;
+        // CTA c owns items [nitems*c/grid, nitems*(c+1)/grid) of the tile-major list: the CTAs that hold
+        // a piece of a tile's image are consecutive
+        std::vector<int2> tile_ctas(p->pk_ntiles, make_int2(p->grid, -1));
+        for (int c = 0; c < p->grid; ++c) {
+            const long long a0 = nitems * c / p->grid, a1 = nitems * (c + 1) / p->grid;
+            if (a0 >= a1) continue;
+            for (int t = (int)(a0 / npacks); t <= (int)((a1 - 1) / npacks); ++t) {
+                tile_ctas[t].x = std::min(tile_ctas[t].x, c);
+                tile_ctas[t].y = std::max(tile_ctas[t].y, c);
+            }
+        }
+        if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_packrows, packrows.data(), packrows.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_tile_ctas, tile_ctas.data(), tile_ctas.size())) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->grid * T * p->nxp)) != PDM_OK) return rc;
+        for (int i = 0; i < 2; ++i) {
+            if ((rc = dev_alloc(p, &p->d_plane[i], (size_t)nw * p->nxp)) != PDM_OK) return rc;
+            PDM_CUDA(p, cudaMemset(p->d_plane[i], 0, (size_t)nw * p->nxp * sizeof(float2)));
+            if ((rc = make_plane_map(p, &p->tmap_plane[i], p->d_plane[i], p->nxp, nw, BW)) != PDM_OK) return rc;
+        }
     } else {                                                        // PDM_PATH_NAIVE
         p->taps_mode = 1;
         p->threads = 128;
@@ -639,6 +748,46 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         dim3 rg((nx + 255) / 256, nz);
         pdm_reduce_partials<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->n_partial, nz, nx, a.pstride);
         PDM_CUDA(p, cudaGetLastError());
+    } else if (p->path == PDM_PATH_PACKED) {
+        pdm_pack_params a;
+        memset(&a, 0, sizeof(a));
+        a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega; a.half = p->d_half;
+        a.packrows = p->d_packrows;
+        a.nx = nx; a.nxp = p->nxp; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
+        a.qstride = p->qstride; a.half16 = p->half16;
+        a.npacks = p->pk_npacks; a.ntiles = p->pk_ntiles; a.nitems = p->pk_ntiles * p->pk_npacks;
+        a.TX = p->pk_TX; a.H = p->pk_H; a.T = p->pk_T;
+        a.LS = p->pk_LS; a.BW = p->pk_BW; a.nbox = p->pk_nbox; a.cap = p->pk_cap; a.passes = p->pk_passes;
+        a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
+        pack_fn fn = pack_kernel_for(p);
+        // the first depth block reads the caller's P0 through its own TMA descriptor when its rows are
+        // 16-byte aligned (nx even and an aligned base); otherwise P0 is first repacked into a plane
+        CUtensorMap map_p0;
+        int src = -1;                                    // -1: P0, else index of the plane read
+        if (nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) {
+            int rc = make_plane_map(p, &map_p0, P0_dev, nx, nw, p->pk_BW);
+            if (rc != PDM_OK) return rc;
+        } else {
+            dim3 cg((p->nxp + 255) / 256, nw);
+            pdm_pack_copy_in<<<cg, 256, 0, st>>>(P0, p->d_plane[1], nx, p->nxp, nw);
+            src = 1;
+        }
+        if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
+        const int nblocks = (nz + p->pk_T - 1) / p->pk_T;
+        for (int zb = 0; zb < nblocks; ++zb) {
+            const int dst = src < 0 ? 0 : (src ^ 1);
+            a.z0 = zb * p->pk_T; a.Tz = std::min(p->pk_T, nz - a.z0);
+            a.tmap_in = src < 0 ? map_p0 : p->tmap_plane[src];
+            a.Pout = p->d_plane[dst];
+            a.store_plane = zb + 1 < nblocks ? 1 : 0;
+            fn<<<p->grid, p->threads, p->smem_bytes, st>>>(a);
+            dim3 rg((nx + 255) / 256, a.Tz);
+            pdm_pack_reduce<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->d_tile_ctas, p->pk_TX, p->pk_T,
+                                                 a.z0, nx, p->nxp);
+            src = dst;
+        }
+        PDM_CUDA(p, cudaGetLastError());
+        if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[1], st));
     } else {
         dim3 g1((nx + 127) / 128, nw), g2((nx + 127) / 128);
         const float2 *src = P0;

@@ -1,6 +1,7 @@
 // pdm_common.cuh -- plan layout and small device helpers shared by the kernels of libpdm.
 // Product code: csrc/ shares nothing with the CPU checker (test infrastructure) of this repo.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "../../include/pdm.h"
@@ -55,6 +56,11 @@ struct pdm_plan {
     int tile_x, wgroups;  // tiled path
     int cluster_size, cluster_gper, cluster_passes;   // cluster path: CTAs per line, groups per CTA, passes per step
     int taps_in_smem;     // march: 1 = per-omega rows staged in shared memory, 0 = L1/L2 global rows
+    // packed path (kern_pack.cuh): planes [nw][nxp] ping-pong, T depth steps per tile visit
+    int nxp, pk_T, pk_TX, pk_H, pk_LS, pk_BW, pk_nbox, pk_cap, pk_passes, pk_npacks, pk_ntiles;
+    int2 *d_packrows;     // [npacks] table rows a pack can touch
+    int2 *d_tile_ctas;    // [ntiles] first / last CTA that holds a piece of the tile's image
+    CUtensorMap tmap_plane[2];   // TMA descriptors of d_plane[0], d_plane[1]
     double workspace_bytes;
 };
 

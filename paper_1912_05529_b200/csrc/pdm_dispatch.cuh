@@ -5,11 +5,13 @@
 #include "kern_march.cuh"
 #include "kern_tiled.cuh"
 #include "kern_cluster.cuh"
+#include "kern_pack.cuh"
 
 #define PDM_R 8
 typedef void (*march_fn)(const pdm_march_params);
 typedef void (*tiled_fn)(const pdm_tiled_params);
 typedef void (*cluster_fn)(const pdm_cluster_params);
+typedef void (*pack_fn)(const pdm_pack_params);
 
 // filter half-lengths with a fully unrolled, register-tiled instantiation, in three build parts
 #define PDM_L_PART0(X) X(1) X(2) X(3) X(7) X(12)
@@ -36,3 +38,7 @@ cluster_fn pdm_cluster_kernel_asym_part2(int L, bool taps_smem);
 tiled_fn   pdm_tiled_kernel_asym_part0(int L, bool wide);
 tiled_fn   pdm_tiled_kernel_asym_part1(int L, bool wide);
 tiled_fn   pdm_tiled_kernel_asym_part2(int L, bool wide);
+// frequency-packed, temporally blocked x-tiled form (tu_pack.cu, same three parts)
+pack_fn    pdm_pack_kernel_part0(int L, bool sym);
+pack_fn    pdm_pack_kernel_part1(int L, bool sym);
+pack_fn    pdm_pack_kernel_part2(int L, bool sym);

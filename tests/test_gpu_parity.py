@@ -55,7 +55,7 @@ def assert_parity(pdm, cfg, flags=0, ref=None, expect_path=None):
     return rel, mx
 
 
-PATHS = ["naive", "smem_global", "smem_staged", "tiled", "cluster"]
+PATHS = ["naive", "smem_global", "smem_staged", "tiled", "cluster", "packed"]
 
 
 def path_flags(pdm, name):
@@ -63,7 +63,8 @@ def path_flags(pdm, name):
             "smem_global": pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_GLOBAL,
             "smem_staged": pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_SLICE,
             "tiled": pdm.PDM_PATH_TILED,
-            "cluster": pdm.PDM_PATH_CLUSTER}[name]
+            "cluster": pdm.PDM_PATH_CLUSTER,
+            "packed": pdm.PDM_PATH_PACKED}[name]
 
 
 # ---------------------------------------------------------------- every kernel form, small inputs
@@ -174,6 +175,53 @@ def test_tiled_path_with_unaligned_plane_pointer(pdm):
     assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
 
 
+@pytest.mark.parametrize("T", [0, 1, 2, 3, 4, 8])
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps", [
+    ("field", 300, 21, 7, 15),        # nx below one tile, one ragged pack, nz not a multiple of T
+    ("white", 1000, 13, 19, 25),      # 3 packs (the last ragged), 3 x-tiles, every sample its own row
+    ("layers", 2501, 10, 9, 7),       # odd nx: P0 is repacked for TMA; thread-uniform rows
+    ("field", 1900, 9, 16, 35),       # two whole packs; kernel for L = 17
+    ("const", 129, 17, 3, 51),        # halo of 4 groups fetched per side; T*L far beyond the line
+])
+def test_packed_path_matches_oracle_for_every_block_depth(pdm, T, model, nx, nz, nw, ntaps):
+    """T depth steps per tile visit with recomputed halos, 8
+    adjacent frequencies per quarter warp, tiles moved by TMA with zero fill at the edges (R5); forced
+    T = 1, 2, 3, 4, 8 and the default, ragged nx / nw / nz; parity and bit-identical repeats."""
+    import torch
+    cfg = pdm_inputs.random_problem(37, nx, nz, nw, ntaps, model=model)
+    flags = pdm.PDM_PATH_PACKED | (T << pdm.PDM_CTAS_SHIFT)
+    ref = oracle.migrate(cfg)
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        info = plan.info
+        assert info["path"] == pdm.PDM_PATH_PACKED
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(p0).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    rel, mx = errors(a.cpu().numpy(), ref)
+    assert np.isfinite(a.cpu().numpy()).all() and rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info)
+
+
+def test_packed_path_with_unaligned_p0_pointer(pdm):
+    """Even nx but a P0 that is only 8-byte aligned: TMA cannot address it, so the library repacks it
+    into its own plane first; same image bit for bit as the direct descriptor on an aligned P0."""
+    import torch
+    cfg = pdm_inputs.random_problem(29, 2600, 12, 21, 25, model="field")
+    with pdm.Plan.from_config(cfg, pdm.PDM_PATH_PACKED) as plan:
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        store = torch.empty(p0.numel() + 1, dtype=p0.dtype, device="cuda")
+        shifted = store[1:].view(p0.shape)
+        shifted.copy_(p0)
+        assert shifted.data_ptr() % 16 == 8
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(shifted).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    rel, mx = errors(a.cpu().numpy(), oracle.migrate(cfg))
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+
+
 @pytest.mark.parametrize("nx,nz,nw,ntaps,model,csize", [
     (1000, 24, 5, 25, "white", 4),       # 125 groups over 4 CTAs of one warp: ragged last CTA
     (129, 50, 3, 35, "const", 8),        # 17 groups over 8 CTAs: most CTAs of a cluster idle
@@ -211,6 +259,12 @@ def test_asymmetric_tables_run_on_the_general_kernels(pdm, path, model, nx, nz, 
     L = (ntaps - 1) // 2
     assert not np.array_equal(cfg["table"][:, :L][:, ::-1], cfg["table"][:, L + 1:])
     flags = 0 if path == "auto" else path_flags(pdm, path)
+    if path == "packed" and ntaps == 51:
+        # 27 x 16-byte units per unfolded row: one pack's rows do not fit next to the line tiles
+        rc, h = pdm.pdm_create(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"],
+                               cfg["velocity"], cfg["table"], cfg["du"], flags)
+        assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
+        return
     img, info = gpu_migrate(pdm, cfg, flags, want_info=True)
     assert info["table_symmetric"] == 0
     rel, mx = errors(img, oracle.migrate(cfg))
@@ -239,7 +293,7 @@ def test_auto_small_problem_with_a_huge_table_keeps_a_consistent_layout(pdm):
             assert_parity(pdm, cfg, path_flags(pdm, path), ref=ref)
 
 
-@pytest.mark.parametrize("path", ["smem_staged", "smem_global", "tiled", "cluster"])
+@pytest.mark.parametrize("path", ["smem_staged", "smem_global", "tiled", "cluster", "packed"])
 def test_force_general_flag_takes_the_per_output_gather(pdm, path):
     """PDM_FORCE_GENERAL: a warp-uniform model (layers) run through the per-output tap gather must
     give the same image bit for bit as the thread-uniform fast path (same taps, same order)."""
@@ -412,8 +466,10 @@ def test_randomized_parity_over_forms_shapes_and_filter_lengths(pdm):
     rng = np.random.default_rng(2024)
     forms = [0, pdm.PDM_PATH_SMEM, pdm.PDM_PATH_SMEM | pdm.PDM_TAPS_GLOBAL, pdm.PDM_PATH_TILED,
              pdm.PDM_PATH_CLUSTER, pdm.PDM_PATH_CLUSTER | (4 << pdm.PDM_CTAS_SHIFT),
-             pdm.PDM_PATH_CLUSTER | (8 << pdm.PDM_CTAS_SHIFT)]
-    for i in range(48):
+             pdm.PDM_PATH_CLUSTER | (8 << pdm.PDM_CTAS_SHIFT),
+             pdm.PDM_PATH_PACKED, pdm.PDM_PATH_PACKED | (1 << pdm.PDM_CTAS_SHIFT),
+             pdm.PDM_PATH_PACKED | (5 << pdm.PDM_CTAS_SHIFT)]
+    for i in range(64):
         nx = int(rng.choice([1, 7, 8, 9, 63, 64, 65, 255, 257, 700, 1023, 1500, 2049, 3333, 5000]))
         nz = int(rng.integers(1, 24))
         nw = int(rng.choice([1, 2, 5, 37, 150, 310]))
@@ -474,6 +530,7 @@ def test_gpu_path_properties_superposition_mirror_additivity(pdm, path):
     ("smem whole lines", 333, 10, 5, 25, "layers", "smem_staged"),
     ("tiled", 2600, 8, 6, 25, "field", "tiled"),
     ("cluster", 5000, 8, 6, 25, "layers", "cluster"),
+    ("packed", 2600, 9, 20, 15, "field", "packed"),
 ])
 def test_migrate_is_cuda_graph_capturable(pdm, name, nx, nz, nw, ntaps, model, path):
     """pdm_migrate only enqueues work (no allocation, no host sync, no copies): capture it in a CUDA
