@@ -34,20 +34,24 @@
 #define PDM_PACK_NBUF 3
 
 struct alignas(64) pdm_pack_params {
-    CUtensorMap   tmap_in;    // plane read by this depth block: {x, line} of 8-byte samples, box {BW, 1}
-    float2       *Pout;       // [nw][nxp] plane written by the block's last step
-    float        *partial;    // [grid][T][nxp] image tiles of this depth block, per CTA
-    const float  *q;          // [nz][qstride]
-    const float  *omega;      // [nw]
-    const float4 *half;       // [ntab][half16]
-    const int2   *packrows;   // [npacks] {first, last} table row the pack can touch
+    CUtensorMap   tmap_p0;        // the caller's P0 (first depth block, when its rows are 16-byte aligned)
+    CUtensorMap   tmap_plane[2];  // the plan's ping-pong planes: {x, line} of 8-byte samples, box {BW, 1}
+    float2       *plane[2];       // [nw][nxp]
+    float        *partial;        // [2][grid][T][nxp] image tiles per CTA, double-buffered over depth blocks
+    float        *image;          // [nz][nx]
+    const float  *q;              // [nz][qstride]
+    const float  *omega;          // [nw]
+    const float4 *half;           // [ntab][half16]
+    const int2   *packrows;       // [npacks] {first, last} table row the pack can touch
+    const int2   *tile_ctas;      // [ntiles] first / last CTA holding a piece of the tile's image
+    unsigned     *gbar;           // grid barrier counter (zeroed on the stream before the launch)
+    int first_src;                // -1: block 0 reads P0 through tmap_p0; 1: P0 was repacked into plane[1]
     int nx, nxp, nz, nw, ntab, qstride, half16;
     int npacks, ntiles, nitems;
-    int TX, H, T, z0, Tz;     // outputs per tile, halo of recomputed samples per side, steps per block
-    int LS, BW, nbox;         // line stride (samples), TMA box width, boxes per line
-    int cap;                  // table rows the slice buffer holds
-    int passes;               // groups per thread and step
-    int store_plane;          // 0 on the last depth block (nothing reads the plane any more)
+    int TX, H, T;                 // outputs per tile, recomputed halo per side, depth steps per block
+    int LS, BW, nbox;             // line stride (samples), TMA box width, boxes per line
+    int cap;                      // table rows the slice buffer holds
+    int passes;                   // groups per thread and step
     int force_general;
 };
 
@@ -84,8 +88,8 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
     extern __shared__ __align__(128) unsigned char pdm_pack_smem[];
     __shared__ __align__(8) unsigned long long mbar[2];
     // A4 without a CTA barrier (as in kern_march.cuh): prog[1 + w] = depth steps warp w has completed
-    // since the kernel started, counted THROUGH the items.  A warp owns 4*passes contiguous groups
-    // (32*passes samples >= the filter half-length), so step s+1 of warp w reads only what warps
+    // since the kernel started, counted THROUGH items and depth blocks.  A warp owns 4*passes contiguous
+    // groups (32*passes samples >= the filter half-length), so step s+1 of warp w reads only what warps
     // w-1, w, w+1 wrote in step s and may start as soon as both neighbours have completed step s;
     // that also orders the overwrite of the ping-pong buffer.  prog[0], prog[nwarps+1]: sentinels.
     __shared__ int prog[MAXW + 2];
@@ -93,9 +97,11 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
 
     const int tid = threadIdx.x, NT = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = NT >> 5;
     const int l = lane & 7;                              // line of the pack this lane works on
+    // this CTA's items of EVERY depth block (tile-major list, pack fastest): the same (tile, pack) pairs
+    // each time, so staged table rows survive from block to block when they all fit
     const int i0 = (int)((long long)p.nitems * blockIdx.x / gridDim.x);
     const int i1 = (int)((long long)p.nitems * (blockIdx.x + 1) / gridDim.x);
-    if (i0 >= i1) return;
+    const int nmine = i1 - i0;
 
     unsigned char *sm = pdm_pack_smem + ((128u - (pdm_smem_u32(pdm_pack_smem) & 127u)) & 127u);
     const int buf_samples = W * p.LS;
@@ -114,200 +120,230 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
     }
     __syncthreads();
 
-    // Line buffers: 0 and 2 alternate as the LOADED buffer of consecutive items, 1 is the scratch half
-    // of the ping-pong.  TMA: 8 lines x nbox boxes of item (i0 + k) into buffer 2*(k & 1); line l2 starts
-    // 2*l2 samples earlier, so sample x of line l2 lands at l2*LS + (x - X0) + 2*l2.
-    auto issue = [&](int k) {
-        const int item = i0 + k;
-        const int tile = item / p.npacks, pack = item - tile * p.npacks;
-        const int X0 = tile * p.TX - p.H - R * HG;
-        const unsigned bar = pdm_smem_u32(&mbar[k & 1]);
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // generic-proxy accesses of the buffer are done
-        pdm_mbar_expect_tx(bar, (unsigned)(W * p.nbox * p.BW * (int)sizeof(float2)));
-        const unsigned dst0 = pdm_smem_u32(bufs + (size_t)(2 * (k & 1)) * buf_samples);
-        for (int l2 = 0; l2 < W; ++l2)
-            for (int bx = 0; bx < p.nbox; ++bx)
-                pdm_tma_load_2d(dst0 + (unsigned)((l2 * p.LS + bx * p.BW) * (int)sizeof(float2)), &p.tmap_in,
-                                X0 - 2 * l2 + bx * p.BW, pack * W + l2, bar);
-    };
-    if (tid == 0) {
-        issue(0);
-        if (i0 + 1 < i1) issue(1);
-    }
-
     const int ntab_m1 = p.ntab - 1;
     const int gc0 = p.H / R, gc1 = gc0 + p.TX / R;       // groups whose outputs belong to this tile
-    int tile = i0 / p.npacks, pack = i0 - tile * p.npacks;
-    int cur_tile = -1, st_lo = 0, st_hi = -1, jlo = 0;   // staged packs [st_lo, st_hi], first staged row
+    const int nblocks = (p.nz + p.T - 1) / p.T;
+    int st_tile = -1, st_lo = 0, st_hi = -1, jlo = 0;    // staged: packs [st_lo, st_hi] of st_tile's run, first row
     int gs = 0;                                          // depth steps this warp has completed
+    int use0 = 0, use1 = 0;                              // loads each line buffer has received in earlier blocks
 
-    // A1 runs a step ahead of A3: the q values of the NEXT (item, step, pass) are requested before the
-    // current group is computed (they come from L2)
-    float qn[R];
-    auto load_q = [&](int tl, int t, int pass) {
-        const int g = (warp * p.passes + pass) * 4 + (lane >> 3);
-        const int xg = tl * p.TX - p.H + R * g;
-        const int xq = min(max(xg, 0), p.qstride - R);
-        const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)(p.z0 + t) * p.qstride + xq);
-        const float4 a = __ldg(qp), b = __ldg(qp + 1);
-        qn[0] = a.x; qn[1] = a.y; qn[2] = a.z; qn[3] = a.w; qn[4] = b.x; qn[5] = b.y; qn[6] = b.z; qn[7] = b.w;
-    };
-    load_q(tile, 0, 0);
+    for (int blk = 0; blk < nblocks; ++blk) {
+        const int z0 = blk * p.T, Tz = min(p.T, p.nz - z0);
+        const bool store_plane = blk + 1 < nblocks;      // nothing reads the last block's plane
+        const CUtensorMap *const tmap = blk == 0 ? (p.first_src < 0 ? &p.tmap_p0 : &p.tmap_plane[1])
+                                                 : &p.tmap_plane[(blk - 1) & 1];
+        float2 *const Pout = p.plane[blk & 1];
+        float *const partial = p.partial + ((size_t)(blk & 1) * gridDim.x + blockIdx.x) * p.T * p.nxp;
 
-    for (int item = i0; item < i1; ++item) {
-        const int k = item - i0;
-        if (tile != cur_tile || pack > st_hi || pack < st_lo) {           // A2 staging (CTA-uniform, rare)
-            __syncthreads();                                              // every warp is done with the old slice
-            if (cur_tile >= 0 && tile != cur_tile) {                      // the CTA leaves a tile: flush its image
-                float *dst = p.partial + (size_t)blockIdx.x * p.T * p.nxp;
-                const int x0 = cur_tile * p.TX;
-                for (int i = tid; i < p.Tz * p.TX; i += NT) {
-                    const int t = i / p.TX, x = x0 + (i - t * p.TX);
-                    if (x < p.nxp) dst[(size_t)t * p.nxp + x] = img[i];
-                }
-            }
-            if (tile != cur_tile) {
-                for (int i = tid; i < p.T * p.TX; i += NT) img[i] = 0.f;
-                cur_tile = tile;
-            }
-            // as many of the CTA's next packs of this tile as the slice buffer holds (their row ranges
-            // overlap almost entirely: the range is set by the velocity spread, not by the pack)
-            const int last = min(p.npacks - 1, pack + (i1 - 1 - item));
-            int pe = pack, jhi = p.packrows[pack].y;
-            jlo = p.packrows[pack].x;
-            while (pe < last) {
-                const int2 n = p.packrows[pe + 1];
-                const int lo2 = min(jlo, n.x), hi2 = max(jhi, n.y);
-                if (hi2 - lo2 + 1 > p.cap) break;
-                jlo = lo2; jhi = hi2; ++pe;
-            }
-            const int n4 = (jhi - jlo + 1) * p.half16;
-            const float4 *src = p.half + (size_t)jlo * p.half16;
-            for (int e = tid; e < n4; e += NT) slice[e] = src[e];
-            st_lo = pack; st_hi = pe;
-            __syncthreads();
+        // Line buffers: 0 and 2 alternate as the LOADED buffer of consecutive items, 1 is the scratch half
+        // of the ping-pong.  TMA: 8 lines x nbox boxes of item i0 + k into buffer 2*(k & 1); line l2 starts
+        // 2*l2 samples earlier, so sample x of line l2 lands at l2*LS + (x - X0) + 2*l2.
+        auto issue = [&](int k) {
+            const int item = i0 + k;
+            const int tl = item / p.npacks, pk = item - tl * p.npacks;
+            const int X0 = tl * p.TX - p.H - R * HG;
+            const unsigned bar = pdm_smem_u32(&mbar[k & 1]);
+            asm volatile("fence.proxy.async;" ::: "memory");          // generic-proxy accesses (buffer, planes) are done
+            pdm_mbar_expect_tx(bar, (unsigned)(W * p.nbox * p.BW * (int)sizeof(float2)));
+            const unsigned dst0 = pdm_smem_u32(bufs + (size_t)(2 * (k & 1)) * buf_samples);
+            for (int l2 = 0; l2 < W; ++l2)
+                for (int bx = 0; bx < p.nbox; ++bx)
+                    pdm_tma_load_2d(dst0 + (unsigned)((l2 * p.LS + bx * p.BW) * (int)sizeof(float2)), tmap,
+                                    X0 - 2 * l2 + bx * p.BW, pk * W + l2, bar);
+        };
+        if (tid == 0 && nmine > 0) {
+            issue(0);
+            if (nmine > 1) issue(1);
         }
-        const int line = pack * W + l;
-        const float w = p.omega[min(line, p.nw - 1)];
-        const int bL = 2 * (k & 1);
-        int tile_n = tile, pack_n = pack + 1;                             // the next item
-        if (pack_n == p.npacks) { pack_n = 0; ++tile_n; }
 
-        pdm_mbar_wait(pdm_smem_u32(&mbar[k & 1]), (unsigned)(k >> 1) & 1u);   // this item's tiles have landed
+        int tile = i0 / p.npacks, pack = i0 - tile * p.npacks;
+        int cur_tile = -1;                               // tile whose image the CTA is accumulating
+        // A1 runs a step ahead of A3: the q values of the NEXT (item, step, pass) are requested before
+        // the current group is computed (they come from L2)
+        float qn[R];
+        auto load_q = [&](int tl, int t, int pass) {
+            const int g = (warp * p.passes + pass) * 4 + (lane >> 3);
+            const int xg = tl * p.TX - p.H + R * g;
+            const int xq = min(max(xg, 0), p.qstride - R);
+            const float4 *qp = reinterpret_cast<const float4 *>(p.q + (size_t)(z0 + t) * p.qstride + xq);
+            const float4 a = __ldg(qp), b = __ldg(qp + 1);
+            qn[0] = a.x; qn[1] = a.y; qn[2] = a.z; qn[3] = a.w; qn[4] = b.x; qn[5] = b.y; qn[6] = b.z; qn[7] = b.w;
+        };
+        if (nmine > 0) load_q(tile, 0, 0);
 
-        for (int t = 0; t < p.Tz; ++t) {
-            const float2 *cur = bufs + (size_t)((t & 1) ? 1 : bL) * buf_samples;
-            float2 *nxt = bufs + (size_t)((t & 1) ? bL : 1) * buf_samples;
-            const bool last_step = t == p.Tz - 1;
-            for (int pass = 0; pass < p.passes; ++pass) {
-                const int g = (warp * p.passes + pass) * 4 + (lane >> 3);
-                const int xg = tile * p.TX - p.H + R * g;
-                int toff[R];
-                bool un = true;
-#pragma unroll
-                for (int r = 0; r < R; ++r) {                           // A1
-                    const int j = pdm_index(w, qn[r], ntab_m1);
-                    toff[r] = (j - jlo) * p.half16;
-                    un = un && (toff[r] == toff[0]);
-                }
-                const bool uni = __all_sync(0xffffffffu, un && !p.force_general);
-                {                                                       // request the next group's q
-                    int t2 = t, ps2 = pass + 1, tl2 = tile;
-                    bool more = true;
-                    if (ps2 == p.passes) { ps2 = 0; ++t2; }
-                    if (t2 == p.Tz) { t2 = 0; tl2 = tile_n; more = item + 1 < i1; }
-                    if (more) load_q(tl2, t2, ps2);
-                }
-                if (pass == 0 && gs > 0) {                              // A4: neighbours have completed step gs-1
-                    if (lane == 0) {
-                        while (*(volatile int *)&prog[warp] < gs) { }
-                        while (*(volatile int *)&prog[warp + 2] < gs) { }
-                        __threadfence_block();
+        for (int k = 0; k < nmine; ++k) {
+            const bool new_tile = tile != cur_tile;
+            if (new_tile || tile != st_tile || pack > st_hi || pack < st_lo) {   // CTA-uniform, rare
+                __syncthreads();                                          // every warp is done with the old slice / tile
+                if (new_tile) {
+                    if (cur_tile >= 0) {                                  // the CTA leaves a tile: flush its image
+                        const int x0 = cur_tile * p.TX;
+                        for (int i = tid; i < Tz * p.TX; i += NT) {
+                            const int t = i / p.TX, x = x0 + (i - t * p.TX);
+                            if (x < p.nxp) partial[(size_t)t * p.nxp + x] = img[i];
+                        }
                     }
-                    __syncwarp();
+                    for (int i = tid; i < p.T * p.TX; i += NT) img[i] = 0.f;
+                    cur_tile = tile;
                 }
-                const int soff = l * p.LS + R * HG + R * g + 2 * l;
-                const float2 *base = cur + soff;
-                float2 out[R];
-                if (SYM) {
-                    if (uni) pdm_fir_group<L, R, true, false, 0u, 0>(base, slice, toff, out);
-                    else     pdm_fir_group<L, R, false, false, 0u, 0>(base, slice, toff, out);
-                } else {
-                    if (uni) pdm_fir_group_asym<L, R, true, 0>(base, slice, toff, out);
-                    else     pdm_fir_group_asym<L, R, false, 0>(base, slice, toff, out);
-                }
-#pragma unroll
-                for (int r = 0; r < R; ++r)                             // R5: zero outside [0,nx)
-                    if ((unsigned)(xg + r) >= (unsigned)p.nx) out[r] = make_float2(0.f, 0.f);
-                const bool central = g >= gc0 && g < gc1;
-                if (!last_step) {
-                    float2 *dst = nxt + soff;
-#pragma unroll
-                    for (int i = 0; i < R / 2; ++i)
-                        *reinterpret_cast<float4 *>(dst + 2 * i) = make_float4(out[2 * i].x, out[2 * i].y, out[2 * i + 1].x, out[2 * i + 1].y);
-                } else if (p.store_plane && central && xg < p.nxp && line < p.nw) {
-                    float4 *dst = reinterpret_cast<float4 *>(p.Pout + (size_t)line * p.nxp + xg);
-#pragma unroll
-                    for (int i = 0; i < R / 2; ++i)
-                        __stcg(dst + i, make_float4(out[2 * i].x, out[2 * i].y, out[2 * i + 1].x, out[2 * i + 1].y));
-                }
-                // A5: sum Re P over the 8 lines of the pack (fixed tree), lane l ends with output r = l
-                float s;
-                {
-                    float a4[4], a2[2];
-                    const bool b2 = l & 4, b1 = l & 2, b0 = l & 1;
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const float keep = b2 ? out[i + 4].x : out[i].x, send = b2 ? out[i].x : out[i + 4].x;
-                        a4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+                if (tile != st_tile || pack > st_hi || pack < st_lo) {    // A2 staging
+                    // as many of the CTA's next packs of this tile as the slice buffer holds (their row
+                    // ranges overlap almost entirely: the velocity spread sets the range, not the pack)
+                    const int last = min(p.npacks - 1, pack + (nmine - 1 - k));
+                    int pe = pack, jhi = p.packrows[pack].y;
+                    jlo = p.packrows[pack].x;
+                    while (pe < last) {
+                        const int2 n = p.packrows[pe + 1];
+                        const int lo2 = min(jlo, n.x), hi2 = max(jhi, n.y);
+                        if (hi2 - lo2 + 1 > p.cap) break;
+                        jlo = lo2; jhi = hi2; ++pe;
                     }
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        const float keep = b1 ? a4[i + 2] : a4[i], send = b1 ? a4[i] : a4[i + 2];
-                        a2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
-                    }
-                    const float keep = b0 ? a2[1] : a2[0], send = b0 ? a2[0] : a2[1];
-                    s = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+                    const int n4 = (jhi - jlo + 1) * p.half16;
+                    const float4 *src = p.half + (size_t)jlo * p.half16;
+                    for (int e = tid; e < n4; e += NT) slice[e] = src[e];
+                    st_tile = tile; st_lo = pack; st_hi = pe;
                 }
-                if (central) img[t * p.TX + (g - gc0) * R + l] += s;
+                __syncthreads();
             }
-            ++gs;
-            __syncwarp();                                               // A4: publish this warp's step
+            const int line = pack * W + l;
+            const float w = p.omega[min(line, p.nw - 1)];
+            const int jloh = jlo * p.half16;
+            const int bL = 2 * (k & 1);
+            const int uses = ((k & 1) ? use1 : use0) + (k >> 1);          // earlier loads of this buffer
+            int tile_n = tile, pack_n = pack + 1;                         // the next item
+            if (pack_n == p.npacks) { pack_n = 0; ++tile_n; }
+
+            pdm_mbar_wait(pdm_smem_u32(&mbar[k & 1]), (unsigned)uses & 1u);   // this item's tiles have landed
+
+            for (int t = 0; t < Tz; ++t) {
+                const float2 *cur = bufs + (size_t)((t & 1) ? 1 : bL) * buf_samples;
+                float2 *nxt = bufs + (size_t)((t & 1) ? bL : 1) * buf_samples;
+                const bool last_step = t == Tz - 1;
+                for (int pass = 0; pass < p.passes; ++pass) {
+                    const int g = (warp * p.passes + pass) * 4 + (lane >> 3);
+                    const int xg = tile * p.TX - p.H + R * g;
+                    int toff[R];
+                    bool un = true;
+#pragma unroll
+                    for (int r = 0; r < R; ++r) {                       // A1
+                        toff[r] = pdm_index(w, qn[r], ntab_m1) * p.half16 - jloh;
+                        un = un && (toff[r] == toff[0]);
+                    }
+                    const bool uni = __all_sync(0xffffffffu, un && !p.force_general);
+                    {                                                   // request the next group's q
+                        int t2 = t, ps2 = pass + 1, tl2 = tile;
+                        bool more = true;
+                        if (ps2 == p.passes) { ps2 = 0; ++t2; }
+                        if (t2 == Tz) { t2 = 0; tl2 = tile_n; more = k + 1 < nmine; }
+                        if (more) load_q(tl2, t2, ps2);
+                    }
+                    if (pass == 0 && gs > 0) {                          // A4: neighbours have completed step gs-1
+                        if (lane == 0) {
+                            while (*(volatile int *)&prog[warp] < gs) { }
+                            while (*(volatile int *)&prog[warp + 2] < gs) { }
+                            __threadfence_block();
+                        }
+                        __syncwarp();
+                    }
+                    const int soff = l * p.LS + R * HG + R * g + 2 * l;
+                    const float2 *base = cur + soff;
+                    float2 out[R];
+                    if (SYM) {
+                        if (uni) pdm_fir_group<L, R, true, false, 0u, 0>(base, slice, toff, out);
+                        else     pdm_fir_group<L, R, false, false, 0u, 0>(base, slice, toff, out);
+                    } else {
+                        if (uni) pdm_fir_group_asym<L, R, true, 0>(base, slice, toff, out);
+                        else     pdm_fir_group_asym<L, R, false, 0>(base, slice, toff, out);
+                    }
+                    if (xg < 0 || xg + R > p.nx) {                      // R5: zero outside [0,nx) (edge groups only)
+#pragma unroll
+                        for (int r = 0; r < R; ++r)
+                            if ((unsigned)(xg + r) >= (unsigned)p.nx) out[r] = make_float2(0.f, 0.f);
+                    }
+                    const bool central = g >= gc0 && g < gc1;
+                    if (!last_step) {
+                        float2 *dst = nxt + soff;
+#pragma unroll
+                        for (int i = 0; i < R / 2; ++i)
+                            *reinterpret_cast<float4 *>(dst + 2 * i) = make_float4(out[2 * i].x, out[2 * i].y, out[2 * i + 1].x, out[2 * i + 1].y);
+                    } else if (store_plane && central && xg < p.nxp && line < p.nw) {
+                        float4 *dst = reinterpret_cast<float4 *>(Pout + (size_t)line * p.nxp + xg);
+#pragma unroll
+                        for (int i = 0; i < R / 2; ++i)
+                            __stcg(dst + i, make_float4(out[2 * i].x, out[2 * i].y, out[2 * i + 1].x, out[2 * i + 1].y));
+                    }
+                    // A5: sum Re P over the 8 lines of the pack (fixed tree), lane l ends with output r = l
+                    float s;
+                    {
+                        float a4[4], a2[2];
+                        const bool b2 = l & 4, b1 = l & 2, b0 = l & 1;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const float keep = b2 ? out[i + 4].x : out[i].x, send = b2 ? out[i].x : out[i + 4].x;
+                            a4[i] = keep + __shfl_xor_sync(0xffffffffu, send, 4);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 2; ++i) {
+                            const float keep = b1 ? a4[i + 2] : a4[i], send = b1 ? a4[i] : a4[i + 2];
+                            a2[i] = keep + __shfl_xor_sync(0xffffffffu, send, 2);
+                        }
+                        const float keep = b0 ? a2[1] : a2[0], send = b0 ? a2[0] : a2[1];
+                        s = keep + __shfl_xor_sync(0xffffffffu, send, 1);
+                    }
+                    if (central) img[t * p.TX + (g - gc0) * R + l] += s;
+                }
+                ++gs;
+                __syncwarp();                                           // A4: publish this warp's step
+                if (lane == 0) {
+                    __threadfence_block();
+                    *(volatile int *)&prog[warp + 1] = gs;
+                }
+            }
+            // The warp is done with this item's loaded buffer; the LAST warp to get here refills it with
+            // the tiles of item k+2 (item k+1 is already in flight in the other buffer)
             if (lane == 0) {
                 __threadfence_block();
-                *(volatile int *)&prog[warp + 1] = gs;
+                const bool last_warp = atomicAdd(&buf_done[k & 1], 1) == (uses + 1) * nwarps - 1;
+                if (last_warp && k + 2 < nmine) issue(k + 2);
+            }
+            tile = tile_n; pack = pack_n;
+        }
+        use0 += (nmine + 1) >> 1; use1 += nmine >> 1;
+        __syncthreads();
+        if (cur_tile >= 0) {                                              // flush the last tile's image
+            const int x0 = cur_tile * p.TX;
+            for (int i = tid; i < Tz * p.TX; i += NT) {
+                const int t = i / p.TX, x = x0 + (i - t * p.TX);
+                if (x < p.nxp) partial[(size_t)t * p.nxp + x] = img[i];
             }
         }
-        // The warp is done with this item's loaded buffer; the LAST warp to get here refills it with the
-        // tiles of item k+2 (item k+1 is already in flight in the other buffer)
-        if (lane == 0) {
-            __threadfence_block();
-            const bool last_warp = atomicAdd(&buf_done[k & 1], 1) == ((k >> 1) + 1) * nwarps - 1;
-            if (last_warp && k + 2 < i1 - i0) issue(k + 2);
+        // Depth blocks are ordered by a grid-wide barrier (all CTAs are co-resident: cooperative launch):
+        // the planes and image tiles written above are read by other CTAs (TMA / the reduction) after it
+        asm volatile("fence.proxy.async;" ::: "memory");
+        __threadfence();
+        __syncthreads();
+        if (tid == 0) {
+            const unsigned target = (unsigned)(blk + 1) * gridDim.x;
+            atomicAdd(p.gbar, 1u);
+            unsigned v;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p.gbar) : "memory");
+            } while (v < target);
         }
-        tile = tile_n; pack = pack_n;
-    }
-    __syncthreads();
-    {                                                                     // flush the last tile's image
-        float *dst = p.partial + (size_t)blockIdx.x * p.T * p.nxp;
-        const int x0 = cur_tile * p.TX;
-        for (int i = tid; i < p.Tz * p.TX; i += NT) {
-            const int t = i / p.TX, x = x0 + (i - t * p.TX);
-            if (x < p.nxp) dst[(size_t)t * p.nxp + x] = img[i];
+        __syncthreads();
+        // A5, second half: image rows of this depth block = sum of the CTAs' tiles in CTA order
+        {
+            const float *part = p.partial + (size_t)(blk & 1) * gridDim.x * p.T * p.nxp;
+            const int n = Tz * p.nx;
+            for (int i = blockIdx.x * NT + tid; i < n; i += gridDim.x * NT) {
+                const int t = i / p.nx, x = i - t * p.nx;
+                const int2 c = p.tile_ctas[x / p.TX];
+                float s = 0.f;
+                for (int c2 = c.x; c2 <= c.y; ++c2) s += __ldcg(part + ((size_t)c2 * p.T + t) * p.nxp + x);
+                p.image[(size_t)(z0 + t) * p.nx + x] = s;
+            }
         }
     }
-}
-
-// A5, second half for this path: image rows of one depth block = sum of the CTAs' tiles in CTA order
-static __global__ void pdm_pack_reduce(const float *__restrict__ partial, float *__restrict__ image,
-                                const int2 *__restrict__ tile_ctas, int TX, int T, int z0, int nx, int nxp)
-{
-    const int x = blockIdx.x * blockDim.x + threadIdx.x, t = blockIdx.y;
-    if (x >= nx) return;
-    const int2 c = tile_ctas[x / TX];
-    float s = 0.f;
-    for (int k = c.x; k <= c.y; ++k) s += __ldcs(partial + ((size_t)k * T + t) * nxp + x);
-    image[(size_t)(z0 + t) * nx + x] = s;
 }
 
 // repack of a caller's P0 whose rows TMA cannot address (odd nx or an 8-byte aligned base)

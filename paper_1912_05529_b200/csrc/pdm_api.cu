@@ -622,9 +622,14 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if (nitems > 0x7fffffffLL) return PDM_ERR_UNSUPPORTED;
         p->ctas_per_sm = 1;
         p->grid = (int)std::min<long long>(nitems, p->sm_count);
-        const int nblocks = (nz + T - 1) / T;
-        p->launches = 2 * nblocks;
+        p->launches = 1;
         p->n_partial = p->grid;
+        {
+            int coop = 0, per_sm = 0;
+            PDM_CUDA(p, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device));
+            PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, NT, (size_t)p->smem_bytes));
+            if (!coop || per_sm < 1) return PDM_ERR_UNSUPPORTED;   // the depth blocks need all CTAs co-resident
+        }
         // CTA c owns items [nitems*c/grid, nitems*(c+1)/grid) of the tile-major list: the CTAs that hold
         // a piece of a tile's image are consecutive
         std::vector<int2> tile_ctas(p->pk_ntiles, make_int2(p->grid, -1));
@@ -639,7 +644,8 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_packrows, packrows.data(), packrows.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_tile_ctas, tile_ctas.data(), tile_ctas.size())) != PDM_OK) return rc;
-        if ((rc = dev_alloc(p, &p->d_partial, (size_t)p->grid * T * p->nxp)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_partial, (size_t)2 * p->grid * T * p->nxp)) != PDM_OK) return rc;
+        if ((rc = dev_alloc(p, &p->d_flags, (size_t)1)) != PDM_OK) return rc;
         for (int i = 0; i < 2; ++i) {
             if ((rc = dev_alloc(p, &p->d_plane[i], (size_t)nw * p->nxp)) != PDM_OK) return rc;
             PDM_CUDA(p, cudaMemset(p->d_plane[i], 0, (size_t)nw * p->nxp * sizeof(float2)));
@@ -751,8 +757,12 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
     } else if (p->path == PDM_PATH_PACKED) {
         pdm_pack_params a;
         memset(&a, 0, sizeof(a));
-        a.partial = p->d_partial; a.q = p->d_q; a.omega = p->d_omega; a.half = p->d_half;
-        a.packrows = p->d_packrows;
+        a.tmap_plane[0] = p->tmap_plane[0]; a.tmap_plane[1] = p->tmap_plane[1];
+        a.plane[0] = p->d_plane[0]; a.plane[1] = p->d_plane[1];
+        a.partial = p->d_partial; a.image = image_dev;
+        a.q = p->d_q; a.omega = p->d_omega; a.half = p->d_half;
+        a.packrows = p->d_packrows; a.tile_ctas = p->d_tile_ctas;
+        a.gbar = reinterpret_cast<unsigned *>(p->d_flags);
         a.nx = nx; a.nxp = p->nxp; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
         a.qstride = p->qstride; a.half16 = p->half16;
         a.npacks = p->pk_npacks; a.ntiles = p->pk_ntiles; a.nitems = p->pk_ntiles * p->pk_npacks;
@@ -762,31 +772,23 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         pack_fn fn = pack_kernel_for(p);
         // the first depth block reads the caller's P0 through its own TMA descriptor when its rows are
         // 16-byte aligned (nx even and an aligned base); otherwise P0 is first repacked into a plane
-        CUtensorMap map_p0;
-        int src = -1;                                    // -1: P0, else index of the plane read
         if (nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) {
-            int rc = make_plane_map(p, &map_p0, P0_dev, nx, nw, p->pk_BW);
+            int rc = make_plane_map(p, &a.tmap_p0, P0_dev, nx, nw, p->pk_BW);
             if (rc != PDM_OK) return rc;
+            a.first_src = -1;
         } else {
             dim3 cg((p->nxp + 255) / 256, nw);
             pdm_pack_copy_in<<<cg, 256, 0, st>>>(P0, p->d_plane[1], nx, p->nxp, nw);
-            src = 1;
+            a.tmap_p0 = p->tmap_plane[1];
+            a.first_src = 1;
         }
+        // one launch for all depth blocks: the CTAs synchronise between blocks on a counter in global
+        // memory (cooperative launch = all co-resident), zeroed on the stream first
+        PDM_CUDA(p, cudaMemsetAsync(p->d_flags, 0, sizeof(int), st));
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
-        const int nblocks = (nz + p->pk_T - 1) / p->pk_T;
-        for (int zb = 0; zb < nblocks; ++zb) {
-            const int dst = src < 0 ? 0 : (src ^ 1);
-            a.z0 = zb * p->pk_T; a.Tz = std::min(p->pk_T, nz - a.z0);
-            a.tmap_in = src < 0 ? map_p0 : p->tmap_plane[src];
-            a.Pout = p->d_plane[dst];
-            a.store_plane = zb + 1 < nblocks ? 1 : 0;
-            fn<<<p->grid, p->threads, p->smem_bytes, st>>>(a);
-            dim3 rg((nx + 255) / 256, a.Tz);
-            pdm_pack_reduce<<<rg, 256, 0, st>>>(p->d_partial, image_dev, p->d_tile_ctas, p->pk_TX, p->pk_T,
-                                                 a.z0, nx, p->nxp);
-            src = dst;
-        }
-        PDM_CUDA(p, cudaGetLastError());
+        void *args[] = { (void *)&a };
+        PDM_CUDA(p, cudaLaunchCooperativeKernel((const void *)fn, dim3(p->grid), dim3(p->threads), args,
+                                                (size_t)p->smem_bytes, st));
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[1], st));
     } else {
         dim3 g1((nx + 127) / 128, nw), g2((nx + 127) / 128);
