@@ -445,7 +445,12 @@ def run_sweep(args):
         for nx in pick(args.sweep_nx, SWEEP_NX):
             for nw in pick(args.sweep_nw, SWEEP_NW):
                 cfg = sweep_point(nx, nw, ntaps, model=args.sweep_model)
-                plan = pdm.Plan.from_config(cfg, args.flags)
+                try:
+                    plan = pdm.Plan.from_config(cfg, args.flags)
+                except pdm.PdmError as e:             # a forced kernel form that cannot run this point
+                    print(json.dumps({"workload": f"configs[4] nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} "
+                                                  f"velocity={args.sweep_model}", "error": str(e)}), flush=True)
+                    continue
                 info = plan.info
                 P0 = torch.from_numpy(cfg["P0"]).to(dev)
                 image = torch.empty((cfg["nz"], nx), dtype=torch.float32, device=dev)

@@ -30,7 +30,7 @@
 #include "kern_march.cuh"
 
 #define PDM_PACK_W 8              // lines per pack = lanes of a quarter warp
-#define PDM_PACK_THREADS 512
+#define PDM_PACK_THREADS 512      // default CTA size (also built: 384, 256)
 #define PDM_PACK_NBUF 3
 
 struct alignas(64) pdm_pack_params {
@@ -42,7 +42,8 @@ struct alignas(64) pdm_pack_params {
     const float  *q;              // [nz][qstride]
     const float  *omega;          // [nw]
     const float4 *half;           // [ntab][half16]
-    const int2   *packrows;       // [npacks] {first, last} table row the pack can touch
+    const float2 *packw;          // [npacks] {lowest, highest} omega of the pack
+    const float2 *tileq;          // [nblocks][ntiles] {min, max} q over the samples a tile visit computes
     const int2   *tile_ctas;      // [ntiles] first / last CTA holding a piece of the tile's image
     unsigned     *gbar;           // grid barrier counter (zeroed on the stream before the launch)
     int first_src;                // -1: block 0 reads P0 through tmap_p0; 1: P0 was repacked into plane[1]
@@ -79,12 +80,13 @@ __device__ __forceinline__ void pdm_tma_load_2d(unsigned dst, const CUtensorMap 
                  :: "r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(bar) : "memory");
 }
 
-template <int L, bool SYM>
-__global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __grid_constant__ pdm_pack_params p)
+// NTHREADS = CTA size the instantiation is compiled for (512: 128 registers per thread; 384: 168; 256: 255)
+template <int L, bool SYM, int NTHREADS>
+__global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_constant__ pdm_pack_params p)
 {
     constexpr int R = 8, W = PDM_PACK_W;
     constexpr int HG = pdm_halo_groups<L, R>();
-    constexpr int MAXW = PDM_PACK_THREADS / 32;
+    constexpr int MAXW = NTHREADS / 32;
     extern __shared__ __align__(128) unsigned char pdm_pack_smem[];
     __shared__ __align__(8) unsigned long long mbar[2];
     // A4 without a CTA barrier (as in kern_march.cuh): prog[1 + w] = depth steps warp w has completed
@@ -123,7 +125,7 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
     const int ntab_m1 = p.ntab - 1;
     const int gc0 = p.H / R, gc1 = gc0 + p.TX / R;       // groups whose outputs belong to this tile
     const int nblocks = (p.nz + p.T - 1) / p.T;
-    int st_tile = -1, st_lo = 0, st_hi = -1, jlo = 0;    // staged: packs [st_lo, st_hi] of st_tile's run, first row
+    int st_tile = -1, st_blk = -1, st_lo = 0, st_hi = -1, jlo = 0;   // staged: packs [st_lo, st_hi] of (st_blk, st_tile), first row
     int gs = 0;                                          // depth steps this warp has completed
     int use0 = 0, use1 = 0;                              // loads each line buffer has received in earlier blocks
 
@@ -173,7 +175,8 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
 
         for (int k = 0; k < nmine; ++k) {
             const bool new_tile = tile != cur_tile;
-            if (new_tile || tile != st_tile || pack > st_hi || pack < st_lo) {   // CTA-uniform, rare
+            const bool restage = tile != st_tile || blk != st_blk || pack > st_hi || pack < st_lo;
+            if (new_tile || restage) {                                    // CTA-uniform, rare
                 __syncthreads();                                          // every warp is done with the old slice / tile
                 if (new_tile) {
                     if (cur_tile >= 0) {                                  // the CTA leaves a tile: flush its image
@@ -186,14 +189,21 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
                     for (int i = tid; i < p.T * p.TX; i += NT) img[i] = 0.f;
                     cur_tile = tile;
                 }
-                if (tile != st_tile || pack > st_hi || pack < st_lo) {    // A2 staging
-                    // as many of the CTA's next packs of this tile as the slice buffer holds (their row
-                    // ranges overlap almost entirely: the velocity spread sets the range, not the pack)
+                if (restage) {                                            // A2 staging
+                    // rows this visit can touch: [idx(lowest w, q_min), idx(highest w, q_max)] with q over the
+                    // samples of this (depth block, tile) only -- and as many of the CTA's next packs of the
+                    // tile as the slice buffer holds (the ranges of neighbouring packs overlap almost entirely)
+                    const float2 tq = p.tileq[(size_t)blk * p.ntiles + tile];
+                    auto rows_of = [&](int pk) {
+                        const float2 w2 = p.packw[pk];
+                        return make_int2(pdm_index(w2.x, tq.x, ntab_m1), pdm_index(w2.y, tq.y, ntab_m1));
+                    };
                     const int last = min(p.npacks - 1, pack + (nmine - 1 - k));
-                    int pe = pack, jhi = p.packrows[pack].y;
-                    jlo = p.packrows[pack].x;
+                    const int2 r0 = rows_of(pack);
+                    int pe = pack, jhi = r0.y;
+                    jlo = r0.x;
                     while (pe < last) {
-                        const int2 n = p.packrows[pe + 1];
+                        const int2 n = rows_of(pe + 1);
                         const int lo2 = min(jlo, n.x), hi2 = max(jhi, n.y);
                         if (hi2 - lo2 + 1 > p.cap) break;
                         jlo = lo2; jhi = hi2; ++pe;
@@ -201,7 +211,7 @@ __global__ void __launch_bounds__(PDM_PACK_THREADS, 1) pdm_pack_kernel(const __g
                     const int n4 = (jhi - jlo + 1) * p.half16;
                     const float4 *src = p.half + (size_t)jlo * p.half16;
                     for (int e = tid; e < n4; e += NT) slice[e] = src[e];
-                    st_tile = tile; st_lo = pack; st_hi = pe;
+                    st_tile = tile; st_blk = blk; st_lo = pack; st_hi = pe;
                 }
                 __syncthreads();
             }

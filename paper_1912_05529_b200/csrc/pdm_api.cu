@@ -60,7 +60,7 @@ static void free_plan(pdm_plan *p)
     cudaFree(p->d_plane[0]); cudaFree(p->d_plane[1]); cudaFree(p->d_flags);
     cudaFree(p->d_handoff); cudaFree(p->d_segs); cudaFree(p->d_segoff);
     cudaFree(p->d_stage_p0); cudaFree(p->d_stage_img);
-    cudaFree(p->d_packrows); cudaFree(p->d_tile_ctas);
+    cudaFree(p->d_packw); cudaFree(p->d_tileq); cudaFree(p->d_tile_ctas);
     for (int i = 0; i < 3; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
     delete p;
 }
@@ -185,9 +185,9 @@ static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide)
 }
 static pack_fn pack_kernel_for(const pdm_plan *p)
 {
-    pack_fn f = pdm_pack_kernel_part0(p->Lk, p->sym != 0);
-    if (!f) f = pdm_pack_kernel_part1(p->Lk, p->sym != 0);
-    if (!f) f = pdm_pack_kernel_part2(p->Lk, p->sym != 0);
+    pack_fn f = pdm_pack_kernel_part0(p->Lk, p->sym != 0, p->threads);
+    if (!f) f = pdm_pack_kernel_part1(p->Lk, p->sym != 0, p->threads);
+    if (!f) f = pdm_pack_kernel_part2(p->Lk, p->sym != 0, p->threads);
     return f;
 }
 // TMA descriptor of a [nrows][row_samples] array of 8-byte samples (complex64 moved as opaque 64-bit
@@ -577,41 +577,68 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     } else if (p->path == PDM_PATH_PACKED) {
         // kern_pack.cuh: 8 adjacent frequencies per quarter warp, T depth steps per tile visit
         p->taps_mode = 2;
-        const int NT = PDM_PACK_THREADS, W = PDM_PACK_W;
+        const int W = PDM_PACK_W;
+        const unsigned nsel = (p->flags >> PDM_THREADS_SHIFT) & 0xFFu; // forced CTA size / 32: 8, 12 or 16
+        if (nsel && nsel != 8 && nsel != 12 && nsel != 16) return PDM_ERR_UNSUPPORTED;
         const unsigned tsel = (p->flags >> PDM_CTAS_SHIFT) & 0xFu;     // forced steps per visit
-        // default: the longest T whose recomputed halo stays under ~10 % of the tile
-        int T = tsel ? (int)tsel : (Lk <= 7 ? 4 : (Lk <= 12 ? 3 : 2));
-        T = std::min(T, nz);
-        const int passes = 1;
-        const int TXH = NT / W * R * passes;               // samples a CTA computes per line and step
-        const int H = round_up((T - 1) * Lk, R);           // recomputed halo per side
-        const int TX = TXH - 2 * H;
-        if (TX < 8 * R) return PDM_ERR_UNSUPPORTED;
+        // default: the longest T whose recomputed halo stays near 10 % of the tile
+        const int T = std::min(nz, tsel ? (int)tsel : (Lk <= 7 ? 4 : (Lk <= 12 ? 3 : 2)));
         p->nxp = round_up(nx, R);
-        const int w_load = TXH + 2 * R * HG + 2 * (W - 1); // samples per line incl. fetched halo and the per-line skew
-        const int nbox = (w_load + 255) / 256;
-        const int BW = round_up((w_load + nbox - 1) / nbox, 16);   // 128-byte aligned box starts
-        const int LS = nbox * BW;
-        const size_t lines_bytes = (size_t)PDM_PACK_NBUF * W * LS * sizeof(float2);
-        const size_t img_bytes = (size_t)T * TX * sizeof(float);
         const int npacks = (nw + W - 1) / W;
-        std::vector<int2> packrows(npacks);
-        int maxrows = 0;
+        std::vector<float2> packw(npacks);
         for (int k = 0; k < npacks; ++k) {
             float wlo = INFINITY, whi = 0.f;
             for (int i = k * W; i < std::min(nw, (k + 1) * W); ++i) { wlo = std::min(wlo, omega[i]); whi = std::max(whi, omega[i]); }
-            packrows[k] = make_int2(host_index(wlo, qmin, ntab), host_index(whi, qmax, ntab));
-            maxrows = std::max(maxrows, packrows[k].y - packrows[k].x + 1);
+            packw[k] = make_float2(wlo, whi);
         }
-        const size_t fixed = 128 + lines_bytes + img_bytes;
-        const size_t budget = (size_t)p->smem_optin - 1024;   // the kernel's static shared memory counts too
-        if (fixed >= budget) return PDM_ERR_UNSUPPORTED;
-        int cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
-        if (cap < maxrows) return PDM_ERR_UNSUPPORTED;     // one pack's rows must fit next to the line tiles
-        cap = std::min(cap, ntab);
+        // CTA size: the largest whose line tiles leave room for the table rows one tile visit can touch
+        // (512 threads = 512 samples per line and step; long filters with widely spread rows take 384 or 256)
+        int NT = 0, passes = 0, TXH = 0, H = 0, TX = 0, nbox = 0, BW = 0, LS = 0, ntiles = 0, cap = 0;
+        const int nblocks = (nz + T - 1) / T;
+        std::vector<float2> tileq;
+        size_t fixed = 0;
+        for (int cand = 512; cand >= 256 && !NT; cand -= 128) {
+            if (nsel && cand != 32 * (int)nsel) continue;
+            passes = cand == 256 ? 2 : 1;                  // groups per thread and step
+            TXH = cand / W * R * passes;                   // samples a CTA computes per line and step
+            H = round_up((T - 1) * Lk, R);                 // recomputed halo per side
+            TX = TXH - 2 * H;
+            if (TX < 8 * R) continue;
+            const int w_load = TXH + 2 * R * HG + 2 * (W - 1);   // samples per line incl. fetched halo and the per-line skew
+            nbox = (w_load + 255) / 256;
+            BW = round_up((w_load + nbox - 1) / nbox, 16); // 128-byte aligned box starts
+            LS = nbox * BW;
+            const size_t lines_bytes = (size_t)PDM_PACK_NBUF * W * LS * sizeof(float2);
+            const size_t img_bytes = (size_t)T * TX * sizeof(float);
+            ntiles = (nx + TX - 1) / TX;
+            // q extrema over the samples one tile visit computes (its T depth rows, its outputs and halo;
+            // columns past nx repeat the last q, as in d_q): they bound the table rows the visit can touch
+            tileq.assign((size_t)nblocks * ntiles, make_float2(0.f, 0.f));
+            int maxrows = 0;
+            for (int b = 0; b < nblocks; ++b)
+                for (int t = 0; t < ntiles; ++t) {
+                    const int xa = std::max(0, t * TX - H), xb = std::min(nx - 1, t * TX - H + TXH - 1);
+                    float lo = INFINITY, hi = 0.f;
+                    for (int z = b * T; z < std::min(nz, (b + 1) * T); ++z) {
+                        const float *row = q.data() + (size_t)z * p->qstride;
+                        for (int x = xa; x <= xb; ++x) { lo = std::min(lo, row[x]); hi = std::max(hi, row[x]); }
+                    }
+                    tileq[(size_t)b * ntiles + t] = make_float2(lo, hi);
+                    for (int k = 0; k < npacks; ++k)
+                        maxrows = std::max(maxrows, host_index(packw[k].y, hi, ntab) - host_index(packw[k].x, lo, ntab) + 1);
+                }
+            fixed = 128 + lines_bytes + img_bytes;
+            const size_t budget = (size_t)p->smem_optin - 1024;   // the kernel's static shared memory counts too
+            if (fixed >= budget) continue;
+            cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
+            if (cap < maxrows) continue;                   // one pack's rows must fit next to the line tiles
+            cap = std::min(cap, ntab);
+            NT = cand;
+        }
+        if (!NT) return PDM_ERR_UNSUPPORTED;
         p->pk_T = T; p->pk_TX = TX; p->pk_H = H; p->pk_LS = LS; p->pk_BW = BW; p->pk_nbox = nbox;
         p->pk_cap = cap; p->pk_passes = passes; p->pk_npacks = npacks;
-        p->pk_ntiles = (nx + TX - 1) / TX;
+        p->pk_ntiles = ntiles;
         p->threads = NT;
         p->tile_x = TX;
         p->smem_bytes = (int)(fixed + (size_t)cap * p->half16 * sizeof(float4));
@@ -642,7 +669,8 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
             }
         }
         if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
-        if ((rc = dev_upload(p, &p->d_packrows, packrows.data(), packrows.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_packw, packw.data(), packw.size())) != PDM_OK) return rc;
+        if ((rc = dev_upload(p, &p->d_tileq, tileq.data(), tileq.size())) != PDM_OK) return rc;
         if ((rc = dev_upload(p, &p->d_tile_ctas, tile_ctas.data(), tile_ctas.size())) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)2 * p->grid * T * p->nxp)) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_flags, (size_t)1)) != PDM_OK) return rc;
@@ -761,7 +789,7 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         a.plane[0] = p->d_plane[0]; a.plane[1] = p->d_plane[1];
         a.partial = p->d_partial; a.image = image_dev;
         a.q = p->d_q; a.omega = p->d_omega; a.half = p->d_half;
-        a.packrows = p->d_packrows; a.tile_ctas = p->d_tile_ctas;
+        a.packw = p->d_packw; a.tileq = p->d_tileq; a.tile_ctas = p->d_tile_ctas;
         a.gbar = reinterpret_cast<unsigned *>(p->d_flags);
         a.nx = nx; a.nxp = p->nxp; a.nz = nz; a.nw = nw; a.ntab = p->ntab;
         a.qstride = p->qstride; a.half16 = p->half16;

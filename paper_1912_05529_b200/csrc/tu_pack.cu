@@ -13,12 +13,18 @@
 #define PDM_PART_FN pdm_pack_kernel_part2
 #endif
 
-pack_fn PDM_PART_FN(int L, bool sym)
+template <int NT>
+static pack_fn pick(int L, bool sym)
 {
     switch (L) {
-#define X(LL) case LL: return sym ? pdm_pack_kernel<LL, true> : pdm_pack_kernel<LL, false>;
+#define X(LL) case LL: return sym ? pdm_pack_kernel<LL, true, NT> : pdm_pack_kernel<LL, false, NT>;
         PDM_L_THIS(X)
 #undef X
     default: return nullptr;
     }
+}
+
+pack_fn PDM_PART_FN(int L, bool sym, int threads)
+{
+    return threads == 256 ? pick<256>(L, sym) : threads == 384 ? pick<384>(L, sym) : threads == 512 ? pick<512>(L, sym) : nullptr;
 }
