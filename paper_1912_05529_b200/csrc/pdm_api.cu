@@ -290,6 +290,124 @@ static int make_half_texture(pdm_plan *p, size_t count)
 static int halo_groups(int L, int R) { return (L + 1 + R - 1) / R; }
 static int round_up(int a, int b) { return (a + b - 1) / b * b; }
 
+// Plan of the frequency-packed, temporally blocked form (kern_pack.cuh).  Feasibility (a CTA size whose
+// line tiles leave room for the table rows of one tile visit, cooperative launch) is settled BEFORE anything
+// is allocated, so that AUTO can fall back to another form on PDM_ERR_UNSUPPORTED.
+static int build_packed(pdm_plan *p, const float *omega, const std::vector<float> &q, const std::vector<float4> &half,
+                        int Lk, int HG)
+{
+    const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, R = PDM_R;
+    int rc;
+    // kern_pack.cuh: 8 adjacent frequencies per quarter warp, T depth steps per tile visit
+    p->taps_mode = 2;
+    const int W = PDM_PACK_W;
+    // the tuning bits mean something else for the other forms: read them only when this form is forced
+    const bool forced = (p->flags & PDM_PATH_MASK) == PDM_PATH_PACKED;
+    const unsigned nsel = forced ? (p->flags >> PDM_THREADS_SHIFT) & 0xFFu : 0u;   // CTA size / 32: 8, 12 or 16
+    if (nsel && nsel != 8 && nsel != 12 && nsel != 16) return PDM_ERR_UNSUPPORTED;
+    const unsigned tsel = forced ? (p->flags >> PDM_CTAS_SHIFT) & 0xFu : 0u;       // steps per tile visit
+    // default: the longest T whose recomputed halo stays near 10 % of the tile
+    const int T = std::min(nz, tsel ? (int)tsel : (Lk <= 7 ? 4 : (Lk <= 12 ? 3 : 2)));
+    p->nxp = round_up(nx, R);
+    const int npacks = (nw + W - 1) / W;
+    std::vector<float2> packw(npacks);
+    for (int k = 0; k < npacks; ++k) {
+        float wlo = INFINITY, whi = 0.f;
+        for (int i = k * W; i < std::min(nw, (k + 1) * W); ++i) { wlo = std::min(wlo, omega[i]); whi = std::max(whi, omega[i]); }
+        packw[k] = make_float2(wlo, whi);
+    }
+    // CTA size: the largest whose line tiles leave room for the table rows one tile visit can touch
+    // (512 threads = 512 samples per line and step; long filters with widely spread rows take 384 or 256)
+    int NT = 0, passes = 0, TXH = 0, H = 0, TX = 0, nbox = 0, BW = 0, LS = 0, ntiles = 0, cap = 0;
+    const int nblocks = (nz + T - 1) / T;
+    std::vector<float2> tileq;
+    size_t fixed = 0;
+    for (int cand = 512; cand >= 256 && !NT; cand -= 128) {
+        if (nsel && cand != 32 * (int)nsel) continue;
+        passes = cand == 256 ? 2 : 1;                  // groups per thread and step
+        TXH = cand / W * R * passes;                   // samples a CTA computes per line and step
+        H = round_up((T - 1) * Lk, R);                 // recomputed halo per side
+        TX = TXH - 2 * H;
+        if (TX < 8 * R) continue;
+        const int w_load = TXH + 2 * R * HG + 2 * (W - 1);   // samples per line incl. fetched halo and the per-line skew
+        nbox = (w_load + 255) / 256;
+        BW = round_up((w_load + nbox - 1) / nbox, 16); // 128-byte aligned box starts
+        LS = nbox * BW;
+        const size_t lines_bytes = (size_t)PDM_PACK_NBUF * W * LS * sizeof(float2);
+        const size_t img_bytes = (size_t)T * TX * sizeof(float);
+        ntiles = (nx + TX - 1) / TX;
+        // q extrema over the samples one tile visit computes (its T depth rows, its outputs and halo;
+        // columns past nx repeat the last q, as in d_q): they bound the table rows the visit can touch
+        tileq.assign((size_t)nblocks * ntiles, make_float2(0.f, 0.f));
+        int maxrows = 0;
+        for (int b = 0; b < nblocks; ++b)
+            for (int t = 0; t < ntiles; ++t) {
+                const int xa = std::max(0, t * TX - H), xb = std::min(nx - 1, t * TX - H + TXH - 1);
+                float lo = INFINITY, hi = 0.f;
+                for (int z = b * T; z < std::min(nz, (b + 1) * T); ++z) {
+                    const float *row = q.data() + (size_t)z * p->qstride;
+                    for (int x = xa; x <= xb; ++x) { lo = std::min(lo, row[x]); hi = std::max(hi, row[x]); }
+                }
+                tileq[(size_t)b * ntiles + t] = make_float2(lo, hi);
+                for (int k = 0; k < npacks; ++k)
+                    maxrows = std::max(maxrows, host_index(packw[k].y, hi, ntab) - host_index(packw[k].x, lo, ntab) + 1);
+            }
+        fixed = 128 + lines_bytes + img_bytes;
+        const size_t budget = (size_t)p->smem_optin - 1024;   // the kernel's static shared memory counts too
+        if (fixed >= budget) continue;
+        cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
+        if (cap < maxrows) continue;                   // one pack's rows must fit next to the line tiles
+        cap = std::min(cap, ntab);
+        NT = cand;
+    }
+    if (!NT) return PDM_ERR_UNSUPPORTED;
+    p->pk_T = T; p->pk_TX = TX; p->pk_H = H; p->pk_LS = LS; p->pk_BW = BW; p->pk_nbox = nbox;
+    p->pk_cap = cap; p->pk_passes = passes; p->pk_npacks = npacks;
+    p->pk_ntiles = ntiles;
+    p->threads = NT;
+    p->tile_x = TX;
+    p->smem_bytes = (int)(fixed + (size_t)cap * p->half16 * sizeof(float4));
+    pack_fn fn = pack_kernel_for(p);
+    if (!fn) return PDM_ERR_UNSUPPORTED;
+    PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
+    const long long nitems = (long long)p->pk_ntiles * npacks;
+    if (nitems > 0x7fffffffLL) return PDM_ERR_UNSUPPORTED;
+    p->ctas_per_sm = 1;
+    p->grid = (int)std::min<long long>(nitems, p->sm_count);
+    p->launches = 1;
+    p->n_partial = p->grid;
+    {
+        int coop = 0, per_sm = 0;
+        PDM_CUDA(p, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device));
+        PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, NT, (size_t)p->smem_bytes));
+        if (!coop || per_sm < 1) return PDM_ERR_UNSUPPORTED;   // the depth blocks need all CTAs co-resident
+    }
+    // CTA c owns items [nitems*c/grid, nitems*(c+1)/grid) of the tile-major list: the CTAs that hold
+    // a piece of a tile's image are consecutive
+    std::vector<int2> tile_ctas(p->pk_ntiles, make_int2(p->grid, -1));
+    for (int c = 0; c < p->grid; ++c) {
+        const long long a0 = nitems * c / p->grid, a1 = nitems * (c + 1) / p->grid;
+        if (a0 >= a1) continue;
+        for (int t = (int)(a0 / npacks); t <= (int)((a1 - 1) / npacks); ++t) {
+            tile_ctas[t].x = std::min(tile_ctas[t].x, c);
+            tile_ctas[t].y = std::max(tile_ctas[t].y, c);
+        }
+    }
+    if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
+    if ((rc = dev_upload(p, &p->d_packw, packw.data(), packw.size())) != PDM_OK) return rc;
+    if ((rc = dev_upload(p, &p->d_tileq, tileq.data(), tileq.size())) != PDM_OK) return rc;
+    if ((rc = dev_upload(p, &p->d_tile_ctas, tile_ctas.data(), tile_ctas.size())) != PDM_OK) return rc;
+    if ((rc = dev_alloc(p, &p->d_partial, (size_t)2 * p->grid * T * p->nxp)) != PDM_OK) return rc;
+    if ((rc = dev_alloc(p, &p->d_flags, (size_t)1)) != PDM_OK) return rc;
+    for (int i = 0; i < 2; ++i) {
+        if ((rc = dev_alloc(p, &p->d_plane[i], (size_t)nw * p->nxp)) != PDM_OK) return rc;
+        PDM_CUDA(p, cudaMemset(p->d_plane[i], 0, (size_t)nw * p->nxp * sizeof(float2)));
+        if ((rc = make_plane_map(p, &p->tmap_plane[i], p->d_plane[i], p->nxp, nw, BW)) != PDM_OK) return rc;
+    }
+    p->path = PDM_PATH_PACKED;
+    return PDM_OK;
+}
+
 static int build_plan(pdm_plan *p, const float *omega, const float *velocity, const pdm_c64 *table)
 {
     const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, ntaps = p->ntaps, L = p->L;
@@ -459,7 +577,26 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     if ((rc = dev_upload(p, &p->d_omega, omega, (size_t)nw)) != PDM_OK) return rc;
     if ((rc = dev_upload(p, &p->d_q, q.data(), q.size())) != PDM_OK) return rc;
 
-    if (p->path == PDM_PATH_SMEM) {
+    // AUTO, models where (nearly) every sample has its own table row: the frequency-packed form makes the
+    // tap gather bank-conflict free when the frequency list is dense against the table (adjacent lines at
+    // most ~1 row apart) and replaces the x-tiled form in any case (measured on configs[4], field model:
+    // 1.06-1.3x over the SMEM form at nx = 4096, 1.2-1.65x over the cluster-pair / x-tiled forms beyond)
+    bool packed_done = false;
+    if (want == PDM_PATH_AUTO && have_L && p->sym && p->contiguous_rows) {
+        float sigma = 0.f;                                  // table rows between adjacent lines of a pack
+        for (int k = 0; k + 1 < nw; ++k)
+            if ((k + 1) % PDM_PACK_W) sigma = std::max(sigma, fabsf(omega[k + 1] - omega[k]) * qmax);
+        const bool dense = nw >= 2 * PDM_PACK_W && sigma <= 1.3f;
+        const long long items = (long long)((nw + PDM_PACK_W - 1) / PDM_PACK_W) * ((nx + 447) / 448);
+        // (sparse lists -- more than ~6 rows between adjacent lines -- keep the x-tiled form: 0.8-0.95x there)
+        if ((p->path == PDM_PATH_TILED && sigma <= 6.f) || (dense && nx >= 3072 && items >= 3LL * p->sm_count)) {
+            rc = build_packed(p, omega, q, half, Lk, HG);
+            if (rc == PDM_OK) packed_done = true;
+            else if (rc != PDM_ERR_UNSUPPORTED) return rc;
+        }
+    }
+    if (packed_done) {
+    } else if (p->path == PDM_PATH_SMEM) {
         if (want_taps == PDM_TAPS_SLICE || want_taps == PDM_TAPS_COMPACT) {
             if (!slice_fits) return PDM_ERR_UNSUPPORTED;
             p->taps_in_smem = 1;
@@ -575,110 +712,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         if ((rc = dev_alloc(p, &p->d_plane[0], (size_t)nw * nx)) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_plane[1], (size_t)nw * nx)) != PDM_OK) return rc;
     } else if (p->path == PDM_PATH_PACKED) {
-        // kern_pack.cuh: 8 adjacent frequencies per quarter warp, T depth steps per tile visit
-        p->taps_mode = 2;
-        const int W = PDM_PACK_W;
-        const unsigned nsel = (p->flags >> PDM_THREADS_SHIFT) & 0xFFu; // forced CTA size / 32: 8, 12 or 16
-        if (nsel && nsel != 8 && nsel != 12 && nsel != 16) return PDM_ERR_UNSUPPORTED;
-        const unsigned tsel = (p->flags >> PDM_CTAS_SHIFT) & 0xFu;     // forced steps per visit
-        // default: the longest T whose recomputed halo stays near 10 % of the tile
-        const int T = std::min(nz, tsel ? (int)tsel : (Lk <= 7 ? 4 : (Lk <= 12 ? 3 : 2)));
-        p->nxp = round_up(nx, R);
-        const int npacks = (nw + W - 1) / W;
-        std::vector<float2> packw(npacks);
-        for (int k = 0; k < npacks; ++k) {
-            float wlo = INFINITY, whi = 0.f;
-            for (int i = k * W; i < std::min(nw, (k + 1) * W); ++i) { wlo = std::min(wlo, omega[i]); whi = std::max(whi, omega[i]); }
-            packw[k] = make_float2(wlo, whi);
-        }
-        // CTA size: the largest whose line tiles leave room for the table rows one tile visit can touch
-        // (512 threads = 512 samples per line and step; long filters with widely spread rows take 384 or 256)
-        int NT = 0, passes = 0, TXH = 0, H = 0, TX = 0, nbox = 0, BW = 0, LS = 0, ntiles = 0, cap = 0;
-        const int nblocks = (nz + T - 1) / T;
-        std::vector<float2> tileq;
-        size_t fixed = 0;
-        for (int cand = 512; cand >= 256 && !NT; cand -= 128) {
-            if (nsel && cand != 32 * (int)nsel) continue;
-            passes = cand == 256 ? 2 : 1;                  // groups per thread and step
-            TXH = cand / W * R * passes;                   // samples a CTA computes per line and step
-            H = round_up((T - 1) * Lk, R);                 // recomputed halo per side
-            TX = TXH - 2 * H;
-            if (TX < 8 * R) continue;
-            const int w_load = TXH + 2 * R * HG + 2 * (W - 1);   // samples per line incl. fetched halo and the per-line skew
-            nbox = (w_load + 255) / 256;
-            BW = round_up((w_load + nbox - 1) / nbox, 16); // 128-byte aligned box starts
-            LS = nbox * BW;
-            const size_t lines_bytes = (size_t)PDM_PACK_NBUF * W * LS * sizeof(float2);
-            const size_t img_bytes = (size_t)T * TX * sizeof(float);
-            ntiles = (nx + TX - 1) / TX;
-            // q extrema over the samples one tile visit computes (its T depth rows, its outputs and halo;
-            // columns past nx repeat the last q, as in d_q): they bound the table rows the visit can touch
-            tileq.assign((size_t)nblocks * ntiles, make_float2(0.f, 0.f));
-            int maxrows = 0;
-            for (int b = 0; b < nblocks; ++b)
-                for (int t = 0; t < ntiles; ++t) {
-                    const int xa = std::max(0, t * TX - H), xb = std::min(nx - 1, t * TX - H + TXH - 1);
-                    float lo = INFINITY, hi = 0.f;
-                    for (int z = b * T; z < std::min(nz, (b + 1) * T); ++z) {
-                        const float *row = q.data() + (size_t)z * p->qstride;
-                        for (int x = xa; x <= xb; ++x) { lo = std::min(lo, row[x]); hi = std::max(hi, row[x]); }
-                    }
-                    tileq[(size_t)b * ntiles + t] = make_float2(lo, hi);
-                    for (int k = 0; k < npacks; ++k)
-                        maxrows = std::max(maxrows, host_index(packw[k].y, hi, ntab) - host_index(packw[k].x, lo, ntab) + 1);
-                }
-            fixed = 128 + lines_bytes + img_bytes;
-            const size_t budget = (size_t)p->smem_optin - 1024;   // the kernel's static shared memory counts too
-            if (fixed >= budget) continue;
-            cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
-            if (cap < maxrows) continue;                   // one pack's rows must fit next to the line tiles
-            cap = std::min(cap, ntab);
-            NT = cand;
-        }
-        if (!NT) return PDM_ERR_UNSUPPORTED;
-        p->pk_T = T; p->pk_TX = TX; p->pk_H = H; p->pk_LS = LS; p->pk_BW = BW; p->pk_nbox = nbox;
-        p->pk_cap = cap; p->pk_passes = passes; p->pk_npacks = npacks;
-        p->pk_ntiles = ntiles;
-        p->threads = NT;
-        p->tile_x = TX;
-        p->smem_bytes = (int)(fixed + (size_t)cap * p->half16 * sizeof(float4));
-        pack_fn fn = pack_kernel_for(p);
-        if (!fn) return PDM_ERR_UNSUPPORTED;
-        PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes));
-        const long long nitems = (long long)p->pk_ntiles * npacks;
-        if (nitems > 0x7fffffffLL) return PDM_ERR_UNSUPPORTED;
-        p->ctas_per_sm = 1;
-        p->grid = (int)std::min<long long>(nitems, p->sm_count);
-        p->launches = 1;
-        p->n_partial = p->grid;
-        {
-            int coop = 0, per_sm = 0;
-            PDM_CUDA(p, cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, p->device));
-            PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, NT, (size_t)p->smem_bytes));
-            if (!coop || per_sm < 1) return PDM_ERR_UNSUPPORTED;   // the depth blocks need all CTAs co-resident
-        }
-        // CTA c owns items [nitems*c/grid, nitems*(c+1)/grid) of the tile-major list: the CTAs that hold
-        // a piece of a tile's image are consecutive
-        std::vector<int2> tile_ctas(p->pk_ntiles, make_int2(p->grid, -1));
-        for (int c = 0; c < p->grid; ++c) {
-            const long long a0 = nitems * c / p->grid, a1 = nitems * (c + 1) / p->grid;
-            if (a0 >= a1) continue;
-            for (int t = (int)(a0 / npacks); t <= (int)((a1 - 1) / npacks); ++t) {
-                tile_ctas[t].x = std::min(tile_ctas[t].x, c);
-                tile_ctas[t].y = std::max(tile_ctas[t].y, c);
-            }
-        }
-        if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
-        if ((rc = dev_upload(p, &p->d_packw, packw.data(), packw.size())) != PDM_OK) return rc;
-        if ((rc = dev_upload(p, &p->d_tileq, tileq.data(), tileq.size())) != PDM_OK) return rc;
-        if ((rc = dev_upload(p, &p->d_tile_ctas, tile_ctas.data(), tile_ctas.size())) != PDM_OK) return rc;
-        if ((rc = dev_alloc(p, &p->d_partial, (size_t)2 * p->grid * T * p->nxp)) != PDM_OK) return rc;
-        if ((rc = dev_alloc(p, &p->d_flags, (size_t)1)) != PDM_OK) return rc;
-        for (int i = 0; i < 2; ++i) {
-            if ((rc = dev_alloc(p, &p->d_plane[i], (size_t)nw * p->nxp)) != PDM_OK) return rc;
-            PDM_CUDA(p, cudaMemset(p->d_plane[i], 0, (size_t)nw * p->nxp * sizeof(float2)));
-            if ((rc = make_plane_map(p, &p->tmap_plane[i], p->d_plane[i], p->nxp, nw, BW)) != PDM_OK) return rc;
-        }
+        if ((rc = build_packed(p, omega, q, half, Lk, HG)) != PDM_OK) return rc;
     } else {                                                        // PDM_PATH_NAIVE
         p->taps_mode = 1;
         p->threads = 128;

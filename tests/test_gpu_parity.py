@@ -313,6 +313,11 @@ def test_auto_policy_picks_the_measured_best_form(pdm):
     assert path_of(16384, 592, 15, "layers")["path"] == pdm.PDM_PATH_CLUSTER    # a line fits a pair of CTAs
     assert path_of(16384, 200, 15, "layers")["path"] == pdm.PDM_PATH_TILED      # ... but 200 lines waste a round
     assert path_of(32768, 400, 15, "layers")["path"] == pdm.PDM_PATH_TILED      # north_star: forced x-tiled
+    # every sample its own table row (profiles/r02_sweep_config4.md)
+    assert path_of(4096, 1024, 15, "field")["path"] == pdm.PDM_PATH_PACKED      # dense frequency list
+    assert path_of(4096, 300, 15, "field")["path"] == pdm.PDM_PATH_SMEM         # too few items for 148 CTAs
+    assert path_of(1024, 2048, 15, "field")["path"] == pdm.PDM_PATH_SMEM        # short lines: tile quantisation
+    assert path_of(32768, 400, 25, "field")["path"] == pdm.PDM_PATH_PACKED      # would be x-tiled otherwise
 
 
 # ---------------------------------------------------------------- BASELINE.json configs
@@ -410,10 +415,10 @@ def test_config4_corners_and_diagonal(pdm, nx, nw, ntaps):
         info = plan.info
         if nx <= 4096:
             assert info["path"] == pdm.PDM_PATH_SMEM or (nw == 64 and info["path"] == pdm.PDM_PATH_CLUSTER), info
-        elif nx == 32768 and nw >= 256:
-            assert info["path"] == pdm.PDM_PATH_TILED, info             # north_star: forced x-tiled
-        elif (nx, nw, ntaps) == (16384, 1024, 15):
-            assert info["path"] == pdm.PDM_PATH_CLUSTER, info           # AUTO's cluster-pair policy
+        elif (nx == 32768 and nw >= 256) or (nx, nw) == (16384, 1024):
+            # per-sample rows, lines too long for one CTA or a frequency list dense against the table:
+            # the frequency-packed, temporally blocked x-tiled form (conflict-free tap gather)
+            assert info["path"] == pdm.PDM_PATH_PACKED, info
         lines = _sample_lines(info, nw)
         assert len(lines) >= min(16, nw)
         full = torch.from_numpy(cfg["P0"]).cuda()
