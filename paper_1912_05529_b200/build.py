@@ -29,7 +29,7 @@ UNITS = [("pdm_api.cu", [], "pdm_api.o"),
          ("tu_cluster.cu", [], "tu_cluster.o"),
          ("tu_tiled.cu", [], "tu_tiled.o")]
 HEADERS = ["pdm_common.cuh", "pdm_dispatch.cuh", "kern_naive.cuh", "kern_peak.cuh", "kern_march.cuh",
-           "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh", "kern_reduce.cuh", "kern_pack.cuh"]
+           "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh", "kern_reduce.cuh", "kern_pack.cuh", "kern_fft.cuh"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC"]
 

@@ -997,17 +997,21 @@ extern "C" int pdm_fp32_peak(int packed, int iters, int repeats, void *cuda_stre
 // time -> frequency transform of the input section
 // ------------------------------------------------------------------------------------------------
 #include "kern_tf.cuh"
+#include "kern_fft.cuh"
 
 struct pdm_tf {
     int nt, nx, nw, device, smem_bytes, warps;
     int *d_bins;
     float2 *d_tw;
+    // nt a power of two: real FFT per trace (kern_fft.cuh); else the contraction (kern_tf.cuh)
+    int fft, log2nt, fft_S, fft_ntw, fft_smem;
+    float2 *d_ftw;
 };
 
 extern "C" int pdm_tf_destroy(pdm_tf *tf)
 {
     if (!tf) return PDM_OK;
-    cudaFree(tf->d_bins); cudaFree(tf->d_tw);
+    cudaFree(tf->d_bins); cudaFree(tf->d_tw); cudaFree(tf->d_ftw);
     delete tf;
     return PDM_OK;
 }
@@ -1049,6 +1053,34 @@ extern "C" int pdm_tf_create(pdm_tf **out, int nt, int nx, int nw, const int *bi
               cudaFuncSetAttribute((const void *)pdm_tf_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                    tf->smem_bytes) == cudaSuccess;
     if (!ok) { cudaGetLastError(); pdm_tf_destroy(tf); return PDM_ERR_CUDA; }
+    if (nt >= 4 && (nt & (nt - 1)) == 0) {                 // power of two: FFT form
+        int lg = 0;
+        while ((1 << lg) < nt) ++lg;
+        std::vector<float2> ftw;                           // per radix-4 stage: (w^j, w^2j, w^3j), w = exp(-2 pi i / M)
+        for (int lm = lg; lm >= 2; lm -= 2) {
+            const int M = 1 << lm, q = M / 4;
+            for (int j = 0; j < q; ++j)
+                for (int r = 1; r <= 3; ++r) {
+                    const double a = two_pi * (double)((long long)r * j % M) / (double)M;
+                    ftw.push_back(make_float2((float)cos(a), (float)(-sin(a))));
+                }
+        }
+        if (ftw.empty()) ftw.push_back(make_float2(1.f, 0.f));
+        const size_t np = (size_t)nt + (nt >> 4) + 1;
+        int S = 16;                                        // pairs of traces per CTA: as many as fit ~160 KB
+        while (S > 1 && (S * np + ftw.size()) * sizeof(float2) > (size_t)160 * 1024) S >>= 1;
+        while (S > 1 && S / 2 >= (nx + 1) / 2) S >>= 1;    // no more pairs than the section has
+        const size_t smem = (S * np + ftw.size()) * sizeof(float2);
+        if (smem <= (size_t)prop.sharedMemPerBlockOptin - 1024 &&
+            cudaMalloc((void **)&tf->d_ftw, ftw.size() * sizeof(float2)) == cudaSuccess &&
+            cudaMemcpy(tf->d_ftw, ftw.data(), ftw.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess &&
+            cudaFuncSetAttribute((const void *)pdm_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                 (int)smem) == cudaSuccess) {
+            tf->fft = 1; tf->log2nt = lg; tf->fft_S = S; tf->fft_ntw = (int)ftw.size(); tf->fft_smem = (int)smem;
+        } else {
+            cudaGetLastError();                            // fall through to the contraction form
+        }
+    }
     // warps per CTA (4 bins each): all tiles take the same time, so pick the CTA height that wastes
     // the least of the last wave
     double best = -1.0;
@@ -1074,6 +1106,19 @@ extern "C" int pdm_tf_forward(pdm_tf *tf, const float *section_dev, pdm_c64 *P0_
     if (!tf || !section_dev || !P0_dev) return PDM_ERR_INVALID_ARG;
     int dev = -1;
     if (cudaGetDevice(&dev) != cudaSuccess || dev != tf->device) { cudaGetLastError(); return PDM_ERR_CUDA; }
+    if (tf->fft) {
+        pdm_fft_params f;
+        f.section = section_dev; f.out = reinterpret_cast<float2 *>(P0_dev);
+        f.bins = tf->d_bins; f.tw = tf->d_ftw;
+        f.nt = tf->nt; f.log2nt = tf->log2nt; f.nx = tf->nx; f.nw = tf->nw;
+        f.S = tf->fft_S; f.ntw = tf->fft_ntw;
+        f.pair_loads = (tf->nx % 2 == 0 && ((uintptr_t)section_dev & 7u) == 0) ? 1 : 0;
+        f.wide_out = (tf->nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) ? 1 : 0;
+        const int per_cta = 2 * tf->fft_S;
+        pdm_fft_kernel<<<(tf->nx + per_cta - 1) / per_cta, PDM_FFT_THREADS, tf->fft_smem, (cudaStream_t)cuda_stream>>>(f);
+        if (cudaGetLastError() != cudaSuccess) return PDM_ERR_CUDA;
+        return PDM_OK;
+    }
     pdm_tf_params a;
     a.section = section_dev; a.out = reinterpret_cast<float2 *>(P0_dev);
     a.bins = tf->d_bins; a.tw = tf->d_tw; a.nt = tf->nt; a.nx = tf->nx; a.nw = tf->nw;

@@ -48,6 +48,11 @@ def gpu_forward(pdm, section, bins):
     (64, 1, [3]),                                          # one trace, one bin
     (4096, 130, list(range(8, 410, 3))),                   # long traces; 2 x-tiles with a 2-sample tail
     (37, 129, list(range(0, 19))),                         # odd nt: every bin of the real spectrum
+    (2048, 77, [0, 1, 5, 300, 1023, 1024]),                # FFT form, odd log2(nt): a last radix-2 stage; odd nx
+    (8192, 36, list(range(100, 1500, 7)) + [4096]),        # longest record: 2 pairs of traces per CTA
+    (32, 1000, list(range(0, 17))),                        # short record: 16 pairs per CTA, every bin
+    (8, 19, [0, 1, 2, 3, 4]),
+    (4, 2, [0, 1, 2]),
 ])
 def test_transform_matches_oracle(pdm, nt, nx, bins):
     rng = np.random.default_rng(nt * 7 + nx)
