@@ -79,7 +79,8 @@ typedef enum {
 #define PDM_NO_BALANCE   (1u << 7)  /* debug: whole lines per CTA (no depth-split load balancing)   */
 #define PDM_REQUIRE_SYMMETRIC (1u << 20) /* refuse a table that is not bitwise symmetric in k        */
                                     /* (PDM_ERR_TABLE_ASYMMETRIC) instead of taking the general kernels */
-#define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto)                   */
+#define PDM_THREADS_SHIFT 8         /* bits 8-15: threads per CTA / 32 (0 = auto); with              */
+                                    /* PDM_PATH_PACKED one of 8, 12, 16 (else PDM_ERR_UNSUPPORTED)  */
 #define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
                                     /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
                                     /* with PDM_PATH_PACKED: depth steps per tile visit T (0 = auto) */
@@ -154,6 +155,12 @@ int pdm_get_info(const pdm_plan *plan, pdm_info *out);
 const char *pdm_strerror(int code);
 
 /*
+ * ================================================================================================
+ * MEASUREMENT / DEBUG entry points -- not part of the hot path's contract; used by
+ * bench.py for the roofline figures and by the tests for pin P12.  Everything above this banner is
+ * the product boundary; pdm_tf_* and pdm_design_table further down are the two setup stages.
+ * ================================================================================================
+ *
  * pdm_profile_enable / pdm_profile_read -- per-kernel device timing for the roofline report.
  * While enabled, pdm_migrate records CUDA events on the caller's stream before the dominant
  * kernel(s) (A1-A4: the marching kernel, or all nz x-tiled step launches), between them and the
