@@ -45,6 +45,12 @@ def _load():
         lib.pdm_oracle_index.argtypes = [ctypes.c_float, ctypes.c_float, ctypes.c_double,
                                          ctypes.c_double, ctypes.c_int]
         lib.pdm_oracle_num_threads.restype = ctypes.c_int
+        lib.pdm_oracle_migrate_shot.restype = ctypes.c_int
+        lib.pdm_oracle_migrate_shot.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p]
         _lib = lib
     return _lib
 
@@ -96,3 +102,29 @@ def migrate_field(cfg: dict, omega_index=None):
     """(image, final wavefield complex128 [nlines, nx]) -- the field after the last depth step."""
     return _run(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dz"], cfg["omega"], cfg["velocity"],
                 cfg["table"], cfg["du"], cfg["P0"], omega_index, True)
+
+
+def migrate_shot(cfg: dict, S0, R0, image=None) -> np.ndarray:
+    """Prestack shot-profile image float64 [nz, nx] (reading R17): both wavefields marched with the
+    looked-up operator (the source with its conjugate), zero-lag cross-correlation imaging.
+    `image`: an earlier float64 image to ADD this shot to (returned, modified in place)."""
+    lib = _load()
+    nx, nz, nw = cfg["nx"], cfg["nz"], cfg["nw"]
+    omega = np.ascontiguousarray(cfg["omega"], dtype=np.float32)
+    velocity = np.ascontiguousarray(cfg["velocity"], dtype=np.float32)
+    table = np.ascontiguousarray(cfg["table"], dtype=np.complex64)
+    S0 = np.ascontiguousarray(S0, dtype=np.complex64)
+    R0 = np.ascontiguousarray(R0, dtype=np.complex64)
+    assert omega.shape == (nw,) and velocity.shape == (nz, nx) and S0.shape == (nw, nx) and R0.shape == (nw, nx)
+    acc = image is not None
+    if acc:
+        assert image.dtype == np.float64 and image.shape == (nz, nx) and image.flags.c_contiguous
+    else:
+        image = np.zeros((nz, nx), dtype=np.float64)
+    ntab, ntaps = table.shape
+    rc = lib.pdm_oracle_migrate_shot(nx, nz, nw, float(cfg["dz"]), omega.ctypes.data, velocity.ctypes.data,
+                                     table.ctypes.data, ntab, ntaps, float(cfg["du"]),
+                                     S0.ctypes.data, R0.ctypes.data, 1 if acc else 0, image.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"pdm_oracle_migrate_shot failed with code {rc}")
+    return image

@@ -186,3 +186,73 @@ int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
     free(q32);
     return failed ? ORACLE_ERR_NOMEM : ORACLE_OK;
 }
+
+/*
+ * Prestack (shot-profile) variant -- PAPER.md:151 ("this work can be easily extended to the
+ * prestack depth migration"); the paper gives no equations for it, so this is reading R17 of
+ * DESIGN.md, the textbook shot-profile scheme built from the SAME step as above:
+ *
+ *   S1  R(0,w,x) = recorded shot gather in f-x, S(0,w,x) = source wavefield at the surface
+ *   S2  per depth step and frequency, with the SAME looked-up row W(idx(w, v(x,z))) for both:
+ *         R(z+dz, x) = sum_k      W_k  R(z, x-k)      (upcoming field continued downward, Eq. (1))
+ *         S(z+dz, x) = sum_k conj(W_k) S(z, x-k)      (downgoing field propagated forward:
+ *                                                      the conjugate operator)
+ *   S3  image[z][x] (+)= sum_w Re( conj(S(z+dz,w,x)) * R(z+dz,w,x) )      (zero-lag
+ *         cross-correlation imaging condition; rows as in R6, edges as in R5, index as in R3)
+ *
+ * image_out is ADDED to when accumulate != 0 (several shots into one image), else overwritten.
+ * Pins (tests/test_oracle_shot_pins.py): brute force on tiny grids (independent triple loop),
+ * delta table closed form, spectral identity for both fields in constant velocity (asymmetric
+ * table), global-phase invariance and real bilinearity, point source + point diffractor focusing.
+ */
+int pdm_oracle_migrate_shot(int nx, int nz, int nw, double dz,
+                            const float *omega, const float *velocity,
+                            const oracle_c64 *table, int ntab, int ntaps, double du,
+                            const oracle_c64 *S0, const oracle_c64 *R0,
+                            int accumulate, double *image_out)
+{
+    if (nx <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0 ||
+        !(du > 0.0) || !omega || !velocity || !table || !S0 || !R0 || !image_out)
+        return ORACLE_ERR_ARG;
+    const int L = (ntaps - 1) / 2;
+    const size_t plane = (size_t)nz * (size_t)nx;
+    float *q32 = (float *)malloc(plane * sizeof(float));
+    double *buf = (double *)malloc(sizeof(double) * 8 * (size_t)nx);
+    if (!q32 || !buf) { free(q32); free(buf); return ORACLE_ERR_NOMEM; }
+    for (size_t i = 0; i < plane; ++i) q32[i] = oracle_q32(dz, velocity[i], du);
+    if (!accumulate)
+        for (size_t i = 0; i < plane; ++i) image_out[i] = 0.0;
+    double *S = buf, *Sn = buf + 2 * (size_t)nx, *R = buf + 4 * (size_t)nx, *Rn = buf + 6 * (size_t)nx;
+    for (int iw = 0; iw < nw; ++iw) {                                   /* fixed frequency order */
+        const float w32 = omega[iw];
+        for (int x = 0; x < nx; ++x) {                                  /* S1 */
+            S[2 * x] = (double)S0[(size_t)iw * nx + x].re; S[2 * x + 1] = (double)S0[(size_t)iw * nx + x].im;
+            R[2 * x] = (double)R0[(size_t)iw * nx + x].re; R[2 * x + 1] = (double)R0[(size_t)iw * nx + x].im;
+        }
+        for (int z = 0; z < nz; ++z) {
+            const float *qrow = q32 + (size_t)z * nx;
+            for (int x = 0; x < nx; ++x) {                              /* S2 */
+                const oracle_c64 *row = table + (size_t)oracle_idx(w32, qrow[x], ntab) * ntaps;
+                double rr = 0.0, ri = 0.0, sr = 0.0, si = 0.0;
+                for (int k = -L; k <= L; ++k) {
+                    int xs = x - k;
+                    if (xs < 0 || xs >= nx) continue;
+                    double wr = (double)row[L + k].re, wi = (double)row[L + k].im;
+                    rr += wr * R[2 * xs] - wi * R[2 * xs + 1];          /*      W_k  * R */
+                    ri += wr * R[2 * xs + 1] + wi * R[2 * xs];
+                    sr += wr * S[2 * xs] + wi * S[2 * xs + 1];          /* conj(W_k) * S */
+                    si += wr * S[2 * xs + 1] - wi * S[2 * xs];
+                }
+                Rn[2 * x] = rr; Rn[2 * x + 1] = ri;
+                Sn[2 * x] = sr; Sn[2 * x + 1] = si;
+            }
+            { double *t = R; R = Rn; Rn = t; t = S; S = Sn; Sn = t; }
+            double *irow = image_out + (size_t)z * nx;                  /* S3 */
+            for (int x = 0; x < nx; ++x)
+                irow[x] += S[2 * x] * R[2 * x] + S[2 * x + 1] * R[2 * x + 1];
+        }
+    }
+    free(buf);
+    free(q32);
+    return ORACLE_OK;
+}
