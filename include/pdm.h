@@ -84,7 +84,10 @@ typedef enum {
 #define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
                                     /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
                                     /* with PDM_PATH_PACKED: depth steps per tile visit T (0 = auto) */
-#define PDM_FLAGS_VALID  0x001FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
+#define PDM_PRESTACK      (1u << 21) /* plan for pdm_migrate_shot (shot-profile prestack migration,    */
+                                    /* PAPER.md:151): always the PDM_PATH_PACKED form (AUTO or PACKED   */
+                                    /* path bits), any table; pdm_migrate refuses such a plan           */
+#define PDM_FLAGS_VALID  0x003FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
 
 typedef struct {
     int    path;                 /* PDM_PATH_* actually chosen                                      */
@@ -144,6 +147,24 @@ int pdm_migrate(pdm_plan *plan, const pdm_c64 *P0_dev, float *image_dev, void *c
  * Uses staging buffers owned by the plan (allocated on first use: PDM_ERR_NOMEM possible).
  */
 int pdm_migrate_host(pdm_plan *plan, const pdm_c64 *P0_host, float *image_host, void *cuda_stream);
+
+/*
+ * pdm_migrate_shot -- prestack (shot-profile) migration of ONE shot (PAPER.md:151 names the extension;
+ * the scheme is reading R17 of DESIGN.md, built from the same step, Eq. (1)):
+ *     R(z+dz,w,x) = sum_k      W_k(u)  R(z,w,x-k)      recorded field, continued downward
+ *     S(z+dz,w,x) = sum_k conj(W_k(u)) S(z,w,x-k)      source field, propagated forward
+ *     image[z][x] (+)= sum_w Re( conj(S(z+dz,w,x)) R(z+dz,w,x) )     zero-lag cross-correlation
+ * with the plan's velocity, table, index rule (R3), rows (R6, R7) and zero edges (R5).
+ *   plan       created with PDM_PRESTACK.
+ *   src_dev    DEVICE pdm_c64[nw][nx]  source wavefield at z = 0, read-only.
+ *   rec_dev    DEVICE pdm_c64[nw][nx]  shot gather in f-x at z = 0, read-only.
+ *   image_dev  DEVICE float[nz][nx]    overwritten (accumulate == 0) or added to (accumulate != 0:
+ *                                      several shots into one image, in call order).
+ * Enqueue only, deterministic, one call in flight per plan -- as pdm_migrate.
+ * Errors: PDM_ERR_INVALID_ARG (NULL, a plan without PDM_PRESTACK), PDM_ERR_CUDA.
+ */
+int pdm_migrate_shot(pdm_plan *plan, const pdm_c64 *src_dev, const pdm_c64 *rec_dev, float *image_dev,
+                     int accumulate, void *cuda_stream);
 
 /* pdm_destroy -- free all device and host state of the plan.  NULL is allowed. */
 int pdm_destroy(pdm_plan *plan);

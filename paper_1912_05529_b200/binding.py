@@ -24,10 +24,10 @@ PDM_ERR_CUDA = -6
 
 PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER, PDM_PATH_PACKED = 0, 1, 2, 3, 4, 5
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
-PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC = 1 << 6, 1 << 7, 1 << 20
+PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC, PDM_PRESTACK = 1 << 6, 1 << 7, 1 << 20, 1 << 21
 PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16
 
-EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_destroy", "pdm_get_info",
+EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_migrate_shot", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
                     "pdm_profile_enable", "pdm_profile_read",
                     "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy", "pdm_design_table")
@@ -75,6 +75,8 @@ def load_library(path: str | None = None):
     lib.pdm_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, cf, cf, vp, vp, vp, ci, ci, cd, cu]
     lib.pdm_migrate.restype = ci
     lib.pdm_migrate.argtypes = [vp, vp, vp, vp]
+    lib.pdm_migrate_shot.restype = ci
+    lib.pdm_migrate_shot.argtypes = [vp, vp, vp, vp, ci, vp]
     lib.pdm_migrate_host.restype = ci
     lib.pdm_migrate_host.argtypes = [vp, vp, vp, vp]
     lib.pdm_destroy.restype = ci
@@ -134,6 +136,13 @@ def pdm_create(nx, nz, nw, dx, dz, omega, velocity, table, tab_du, flags=0):
 def pdm_migrate(plan, P0_dev_ptr: int, image_dev_ptr: int, cuda_stream: int = 0) -> int:
     return load_library().pdm_migrate(plan, ctypes.c_void_p(P0_dev_ptr), ctypes.c_void_p(image_dev_ptr),
                                       ctypes.c_void_p(cuda_stream))
+
+
+def pdm_migrate_shot(plan, src_dev_ptr: int, rec_dev_ptr: int, image_dev_ptr: int, accumulate: bool = False,
+                     cuda_stream: int = 0) -> int:
+    return int(load_library().pdm_migrate_shot(plan, ctypes.c_void_p(src_dev_ptr), ctypes.c_void_p(rec_dev_ptr),
+                                               ctypes.c_void_p(image_dev_ptr), 1 if accumulate else 0,
+                                               ctypes.c_void_p(cuda_stream)))
 
 
 def pdm_migrate_host(plan, P0_host_ptr: int, image_host_ptr: int, cuda_stream: int = 0) -> int:
@@ -293,6 +302,27 @@ class Plan:
         rc = pdm_migrate(self._h, P0.data_ptr(), image.data_ptr(), st)
         if rc != PDM_OK:
             raise PdmError(rc, "pdm_migrate")
+        return image
+
+    def migrate_shot(self, src, rec, image=None, accumulate=False, stream=None):
+        """One prestack shot (plan created with PDM_PRESTACK): src, rec torch.complex64 CUDA [nw, nx] ->
+        image float32 CUDA [nz, nx], overwritten or (accumulate) added to."""
+        import torch
+        for t in (src, rec):
+            if not (t.is_cuda and t.dtype == torch.complex64 and t.is_contiguous()
+                    and tuple(t.shape) == (self.nw, self.nx)):
+                raise ValueError("src and rec must be contiguous CUDA complex64 tensors [nw, nx]")
+        if image is None:
+            if accumulate:
+                raise ValueError("accumulate needs an image to add to")
+            image = torch.empty((self.nz, self.nx), dtype=torch.float32, device=rec.device)
+        elif not (image.is_cuda and image.dtype == torch.float32 and image.is_contiguous()
+                  and tuple(image.shape) == (self.nz, self.nx)):
+            raise ValueError("image must be a contiguous CUDA float32 tensor [nz, nx]")
+        st = (stream or torch.cuda.current_stream(rec.device)).cuda_stream
+        rc = pdm_migrate_shot(self._h, src.data_ptr(), rec.data_ptr(), image.data_ptr(), accumulate, st)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm_migrate_shot")
         return image
 
     def migrate_section(self, transform: "SectionTransform", section, image=None, stream=None):

@@ -22,8 +22,11 @@
 //   * sums Re P over the pack with a 3-stage transposing butterfly (7 SHFL) and accumulates the image
 //     tile of its run of packs in shared memory; the last step's samples go from registers to the
 //     output plane.
-// One launch per depth block (the grid-wide dependence between blocks is the launch boundary, as in
-// PAPER.md:85), followed by a fixed-order reduction of the CTAs' image tiles (deterministic).
+// ONE cooperative launch per migration: a CTA owns the same (tile, pack) items in every depth block;
+// blocks are separated by a grid-wide barrier (the paper used kernel exit), after
+// which the CTAs sum the image tiles of the block in fixed CTA order (deterministic) into the image.
+// Prestack mode (xcorr, reading R17): the lines are (receiver, conjugated source) pairs of one
+// frequency and the imaging condition is the zero-lag cross-correlation of the pair.
 #pragma once
 #include <cuda.h>
 #include "pdm_common.cuh"
@@ -54,6 +57,9 @@ struct alignas(64) pdm_pack_params {
     int cap;                      // table rows the slice buffer holds
     int passes;                   // groups per thread and step
     int force_general;
+    int xcorr;                    // prestack: lines 2i / 2i+1 are the receiver field and the conjugated source field of
+                                  // frequency i; the image is sum Re(U R) over the pairs instead of sum Re P (R17)
+    int accumulate;               // add to the image instead of overwriting it (several shots)
 };
 
 __device__ __forceinline__ unsigned pdm_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -287,6 +293,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_cons
                     {
                         float a4[4], a2[2];
                         const bool b2 = l & 4, b1 = l & 2, b0 = l & 1;
+                        if (p.xcorr) {                                  // R17: Re(conj(S) R) = Re(U R) of the line pair,
+#pragma unroll                                                          // counted once (on the even lane)
+                            for (int r = 0; r < R; ++r) {
+                                const float px = __shfl_xor_sync(0xffffffffu, out[r].x, 1);
+                                const float py = __shfl_xor_sync(0xffffffffu, out[r].y, 1);
+                                out[r].x = b0 ? 0.f : out[r].x * px - out[r].y * py;
+                            }
+                        }
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             const float keep = b2 ? out[i + 4].x : out[i].x, send = b2 ? out[i].x : out[i + 4].x;
@@ -350,7 +364,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_cons
                 const int2 c = p.tile_ctas[x / p.TX];
                 float s = 0.f;
                 for (int c2 = c.x; c2 <= c.y; ++c2) s += __ldcg(part + ((size_t)c2 * p.T + t) * p.nxp + x);
-                p.image[(size_t)(z0 + t) * p.nx + x] = s;
+                float *o = p.image + (size_t)(z0 + t) * p.nx + x;
+                *o = p.accumulate ? *o + s : s;
             }
         }
     }
@@ -361,4 +376,21 @@ static __global__ void pdm_pack_copy_in(const float2 *__restrict__ P0, float2 *_
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x, line = blockIdx.y;
     if (x < nxp) plane[(size_t)line * nxp + x] = x < nx ? P0[(size_t)line * nx + x] : make_float2(0.f, 0.f);
+}
+
+// prestack (R17): receiver lines and CONJUGATED source lines interleaved into one plane, so that the
+// same operator marches both (conj(S') = sum_k W_k conj(S)(x-k)) and a line pair shares its table rows
+static __global__ void pdm_pack_interleave(const float2 *__restrict__ rec, const float2 *__restrict__ src,
+                                           float2 *__restrict__ plane, int nx, int nxp, int nw)
+{
+    const int x = blockIdx.x * blockDim.x + threadIdx.x, i = blockIdx.y;
+    if (x >= nxp) return;
+    float2 r = make_float2(0.f, 0.f), u = r;
+    if (x < nx) {
+        r = rec[(size_t)i * nx + x];
+        const float2 s = src[(size_t)i * nx + x];
+        u = make_float2(s.x, -s.y);
+    }
+    plane[(size_t)(2 * i) * nxp + x] = r;
+    plane[(size_t)(2 * i + 1) * nxp + x] = u;
 }

@@ -127,9 +127,21 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
     }
     if (prop.major != 10) return PDM_ERR_UNSUPPORTED;
 
+    // prestack plans carry two lines per frequency (receiver field, conjugated source field): R17
+    const bool prestack = (flags & PDM_PRESTACK) != 0;
+    if (prestack && path != PDM_PATH_AUTO && path != PDM_PATH_PACKED) return PDM_ERR_INVALID_ARG;
+    std::vector<float> omega2;
+    if (prestack) {
+        if ((double)2 * nw * (double)nx > 2.0e9) return PDM_ERR_UNSUPPORTED;
+        omega2.resize((size_t)2 * nw);
+        for (int i = 0; i < nw; ++i) omega2[2 * i] = omega2[2 * i + 1] = omega[i];
+        omega = omega2.data();
+        nw *= 2;
+    }
     pdm_plan *p = new (std::nothrow) pdm_plan();
     if (!p) return PDM_ERR_NOMEM;
     memset(p, 0, sizeof(*p));
+    p->prestack = prestack ? 1 : 0;
     p->nx = nx; p->nz = nz; p->nw = nw; p->ntab = ntab; p->ntaps = ntaps; p->L = L;
     p->dx = dx; p->dz = dz; p->du = tab_du; p->flags = flags;
     p->sym = symmetric ? 1 : 0;
@@ -557,7 +569,10 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;  // (tiled_kernel_for has the same L list)
     if (want == PDM_PATH_PACKED && !have_L) return PDM_ERR_UNSUPPORTED;
-    if (want == PDM_PATH_AUTO)
+    if (p->prestack) {
+        if (!have_L) return PDM_ERR_UNSUPPORTED;
+        p->path = PDM_PATH_PACKED;
+    } else if (want == PDM_PATH_AUTO)
         p->path = (auto_cluster || auto_pair) ? PDM_PATH_CLUSTER
                                : (lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE));
     else p->path = (int)want;
@@ -582,7 +597,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     // most ~1 row apart) and replaces the x-tiled form in any case (measured on configs[4], field model:
     // 1.06-1.3x over the SMEM form at nx = 4096, 1.2-1.65x over the cluster-pair / x-tiled forms beyond)
     bool packed_done = false;
-    if (want == PDM_PATH_AUTO && have_L && p->sym && p->contiguous_rows) {
+    if (want == PDM_PATH_AUTO && !p->prestack && have_L && p->sym && p->contiguous_rows) {
         float sigma = 0.f;                                  // table rows between adjacent lines of a pack
         for (int k = 0; k + 1 < nw; ++k)
             if ((k + 1) % PDM_PACK_W) sigma = std::max(sigma, fabsf(omega[k + 1] - omega[k]) * qmax);
@@ -729,9 +744,19 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
 // ------------------------------------------------------------------------------------------------
 // pdm_migrate: enqueue only -- no allocation, no host sync, no copies (CUDA-graph capturable)
 // ------------------------------------------------------------------------------------------------
+static int migrate_impl(pdm_plan *p, const pdm_c64 *P0_dev, const pdm_c64 *src_dev, float *image_dev,
+                        int accumulate, void *cuda_stream);
+
 extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev, void *cuda_stream)
 {
-    if (!p || !P0_dev || !image_dev) return PDM_ERR_INVALID_ARG;
+    if (!p || !P0_dev || !image_dev || p->prestack) return PDM_ERR_INVALID_ARG;
+    return migrate_impl(p, P0_dev, nullptr, image_dev, 0, cuda_stream);
+}
+
+// P0_dev: the poststack section, or (src_dev != NULL) the receiver field of a prestack shot
+static int migrate_impl(pdm_plan *p, const pdm_c64 *P0_dev, const pdm_c64 *src_dev, float *image_dev,
+                        int accumulate, void *cuda_stream)
+{
     int dev = -1;
     PDM_CUDA(p, cudaGetDevice(&dev));
     if (dev != p->device) { p->last_cuda_error = (int)cudaErrorInvalidDevice; return PDM_ERR_CUDA; }
@@ -834,7 +859,14 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
         pack_fn fn = pack_kernel_for(p);
         // the first depth block reads the caller's P0 through its own TMA descriptor when its rows are
         // 16-byte aligned (nx even and an aligned base); otherwise P0 is first repacked into a plane
-        if (nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) {
+        a.xcorr = p->prestack; a.accumulate = accumulate;
+        if (p->prestack) {                               // (receiver, conj source) line pairs into plane 1
+            dim3 cg((p->nxp + 255) / 256, nw / 2);
+            pdm_pack_interleave<<<cg, 256, 0, st>>>(P0, reinterpret_cast<const float2 *>(src_dev), p->d_plane[1],
+                                                    nx, p->nxp, nw / 2);
+            a.tmap_p0 = p->tmap_plane[1];
+            a.first_src = 1;
+        } else if (nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) {
             int rc = make_plane_map(p, &a.tmap_p0, P0_dev, nx, nw, p->pk_BW);
             if (rc != PDM_OK) return rc;
             a.first_src = -1;
@@ -872,6 +904,13 @@ extern "C" int pdm_migrate(pdm_plan *p, const pdm_c64 *P0_dev, float *image_dev,
     return PDM_OK;
 }
 
+extern "C" int pdm_migrate_shot(pdm_plan *p, const pdm_c64 *src_dev, const pdm_c64 *rec_dev, float *image_dev,
+                                int accumulate, void *cuda_stream)
+{
+    if (!p || !src_dev || !rec_dev || !image_dev || !p->prestack) return PDM_ERR_INVALID_ARG;
+    return migrate_impl(p, rec_dev, src_dev, image_dev, accumulate ? 1 : 0, cuda_stream);
+}
+
 extern "C" int pdm_profile_enable(pdm_plan *p, int enable)
 {
     if (!p) return PDM_ERR_INVALID_ARG;
@@ -893,7 +932,7 @@ extern "C" int pdm_profile_read(pdm_plan *p, float *main_ms, float *reduce_ms)
 
 extern "C" int pdm_migrate_host(pdm_plan *p, const pdm_c64 *P0_host, float *image_host, void *cuda_stream)
 {
-    if (!p || !P0_host || !image_host) return PDM_ERR_INVALID_ARG;
+    if (!p || !P0_host || !image_host || p->prestack) return PDM_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t nP = (size_t)p->nw * p->nx, nI = (size_t)p->nz * p->nx;
     if (!p->d_stage_p0) {
@@ -920,7 +959,7 @@ extern "C" int pdm_get_info(const pdm_plan *p, pdm_info *out)
     if (!p || !out) return PDM_ERR_INVALID_ARG;
     memset(out, 0, sizeof(*out));
     out->path = p->path; out->taps_mode = p->taps_mode;
-    out->nx = p->nx; out->nz = p->nz; out->nw = p->nw; out->ntab = p->ntab; out->ntaps = p->ntaps;
+    out->nx = p->nx; out->nz = p->nz; out->nw = p->prestack ? p->nw / 2 : p->nw; out->ntab = p->ntab; out->ntaps = p->ntaps;
     out->grid_ctas = p->grid; out->threads_per_cta = p->threads; out->ctas_per_sm = p->ctas_per_sm;
     out->smem_bytes = p->smem_bytes; out->launches_per_migrate = p->launches;
     out->sm_count = p->sm_count; out->last_cuda_error = p->last_cuda_error;

@@ -15,6 +15,7 @@ struct pdm_plan {
     double du;
     unsigned flags;
     int path, taps_mode;
+    int prestack;         // PDM_PRESTACK: nw counts LINES = 2 x the caller's frequencies ((receiver, conj source) pairs)
     int sym;              // 1: table bitwise symmetric in k (folded kernels); 0: general kernels (8L+4 lane-ops)
     int device, sm_count, smem_optin;
     int last_cuda_error;

@@ -1,0 +1,89 @@
+"""GPU parity of the prestack (shot-profile) variant, pdm_migrate_shot (
+reading R17), against pdm_oracle_migrate_shot, element by element, at the north_star bar
+(rel-L2 <= 1e-4, per-pixel <= 1e-3 of the image maximum)."""
+import numpy as np
+import pytest
+
+import oracle
+import pdm_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pdm():
+    import torch
+    import paper_1912_05529_b200 as m
+    assert torch.cuda.is_available(), "gpu tests need a B200"
+    m.load_library()
+    return m
+
+
+def _fields(rng, nw, nx):
+    def c():
+        return (rng.standard_normal((nw, nx)) + 1j * rng.standard_normal((nw, nx))).astype(np.complex64)
+    return c(), c()
+
+
+def _errors(got, ref):
+    d = got.astype(np.float64) - ref
+    return np.linalg.norm(d) / np.linalg.norm(ref), np.abs(d).max() / np.abs(ref).max()
+
+
+@pytest.mark.parametrize("T", [0, 1, 3])
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps,sym", [
+    ("field", 300, 21, 7, 15, True),      # 14 lines: one full pack and a ragged one; nx below one tile
+    ("white", 1000, 13, 10, 25, True),    # 3 x-tiles, every sample its own row
+    ("layers", 2501, 10, 5, 7, True),     # odd nx, thread-uniform rows
+    ("field", 700, 9, 8, 31, False),      # asymmetric table: the conjugate operator is NOT the mirrored one
+    ("const", 129, 17, 3, 51, True),
+])
+def test_shot_matches_oracle(pdm, T, model, nx, nz, nw, ntaps, sym):
+    import torch
+    cfg = pdm_inputs.random_problem(53, nx, nz, nw, ntaps, model=model, symmetric=sym)
+    rng = np.random.default_rng(nx + nw)
+    S0, R0 = _fields(rng, nw, nx)
+    ref = oracle.migrate_shot(cfg, S0, R0)
+    flags = pdm.PDM_PRESTACK | ((pdm.PDM_PATH_PACKED | (T << pdm.PDM_CTAS_SHIFT)) if T else 0)
+    with pdm.Plan.from_config(cfg, flags) as plan:
+        info = plan.info
+        assert info["path"] == pdm.PDM_PATH_PACKED and info["nw"] == nw
+        s, r = torch.from_numpy(S0).cuda(), torch.from_numpy(R0).cuda()
+        a = plan.migrate_shot(s, r).clone()
+        b = plan.migrate_shot(s, r).clone()
+        torch.cuda.synchronize()
+        assert torch.equal(a, b)
+        rel, mx = _errors(a.cpu().numpy(), ref)
+        assert rel <= 1e-4 and mx <= 1e-3, (rel, mx, info)
+        # the poststack call is refused on a prestack plan
+        assert pdm.pdm_migrate(plan._h, r.data_ptr(), a.data_ptr(), 0) == pdm.PDM_ERR_INVALID_ARG
+
+
+def test_shots_accumulate_into_one_image(pdm):
+    import torch
+    cfg = pdm_inputs.random_problem(59, 900, 14, 12, 25, model="field")
+    rng = np.random.default_rng(4)
+    shots = [_fields(rng, 12, 900) for _ in range(3)]
+    ref = None
+    for S0, R0 in shots:
+        ref = oracle.migrate_shot(cfg, S0, R0, image=ref)
+    with pdm.Plan.from_config(cfg, pdm.PDM_PRESTACK) as plan:
+        img = None
+        for S0, R0 in shots:
+            img = plan.migrate_shot(torch.from_numpy(S0).cuda(), torch.from_numpy(R0).cuda(), image=img,
+                                    accumulate=img is not None)
+        torch.cuda.synchronize()
+        rel, mx = _errors(img.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx)
+
+
+def test_prestack_argument_errors(pdm):
+    import torch
+    cfg = pdm_inputs.random_problem(61, 200, 5, 4, 15, model="layers")
+    args = (cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"], cfg["velocity"], cfg["table"], cfg["du"])
+    rc, h = pdm.pdm_create(*args, pdm.PDM_PRESTACK | pdm.PDM_PATH_SMEM)     # only the packed form does it
+    assert rc == pdm.PDM_ERR_INVALID_ARG and h is None
+    with pdm.Plan.from_config(cfg, 0) as plan:                              # a poststack plan refuses shots
+        z = torch.zeros((4, 200), dtype=torch.complex64, device="cuda")
+        img = torch.zeros((5, 200), dtype=torch.float32, device="cuda")
+        assert pdm.pdm_migrate_shot(plan._h, z.data_ptr(), z.data_ptr(), img.data_ptr(), False, 0) == pdm.PDM_ERR_INVALID_ARG
