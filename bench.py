@@ -533,6 +533,50 @@ def run_tf(args):
                       "share_of_migration": "compare ms with bench.py's ms_per_step on configs[3]"}), flush=True)
 
 
+# ------------------------------------------------------------------------------- prestack shot
+def run_prestack(args):
+    """one prestack shot (pdm_migrate_shot) on a configs[4] field point -- both
+    wavefields are extrapolated, so a shot counts 2 x nx x nz x nw extrapolated samples."""
+    import torch
+
+    import paper_1912_05529_b200 as pdm
+    from pdm_inputs.configs import sweep_point
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    pdm.load_library()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    nx, nw, ntaps = 4096, 1024, 25
+    cfg = sweep_point(nx, nw, ntaps)
+    rec = torch.from_numpy(cfg["P0"]).to(dev)
+    src = torch.roll(rec, 1, 0).contiguous()
+    image = torch.empty((cfg["nz"], nx), dtype=torch.float32, device=dev)
+    with pdm.Plan.from_config(cfg, pdm.PDM_PRESTACK | args.flags) as plan:
+        info = plan.info
+        for _ in range(max(args.warmup, 3)):
+            plan.migrate_shot(src, rec, image, stream=stream)
+        torch.cuda.synchronize(dev)
+        ms = []
+        for _ in range(args.steps):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            plan.migrate_shot(src, rec, image, stream=stream)
+            b.record(stream)
+            torch.cuda.synchronize(dev)
+            ms.append(a.elapsed_time(b))
+    t = float(np.median(ms)) * 1e-3
+    sps = info["samples"] / t
+    print(json.dumps({"workload": f"prestack shot, configs[4] field nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} "
+                                  "(2 wavefields per frequency)", "kernel": "pdm_pack_kernel (xcorr)",
+                      "path": PATH_NAMES[info["path"]], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
+                      "steps": args.steps, "ms": t * 1e3, "ms_best": float(min(ms)), "samples_per_s": sps,
+                      "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12)}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -545,6 +589,7 @@ def main():
     ap.add_argument("--no-extra", action="store_true",
                     help="skip extra.other_configs (configs[0..2] + two configs[4] points, N = 1 only)")
     ap.add_argument("--tf", action="store_true", help="time the t->f transform of the section (SURVEY 8(f) N1)")
+    ap.add_argument("--prestack", action="store_true", help="time one prestack shot (SURVEY 8(f) N4)")
     ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep, one JSON line per point")
     ap.add_argument("--sweep-taps", default="", help="comma list of tap counts to sweep (default 15,25,51)")
     ap.add_argument("--sweep-nx", default="", help="comma list of nx (default 1024,4096,16384,32768)")
@@ -555,7 +600,7 @@ def main():
     args = ap.parse_args()
     if args.gpus < 1:
         raise SystemExit("bench.py: --gpus must be >= 1")
-    multi = not (args.tf or args.sweep)
+    multi = not (args.tf or args.sweep or args.prestack)
     if multi and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # not under torchrun: start the N ranks ourselves (one process per GPU, NCCL), loudly
         # refusing a box with fewer GPUs -- never a silent 1-rank run that prints n_gpus: 1
@@ -579,6 +624,9 @@ def main():
     if args.tf:
         if rank == 0:
             run_tf(args)
+    elif args.prestack:
+        if rank == 0:
+            run_prestack(args)
     elif args.sweep:
         if rank == 0:
             run_sweep(args)
