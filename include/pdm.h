@@ -84,6 +84,7 @@ typedef enum {
 #define PDM_CTAS_SHIFT    16        /* bits 16-19: CTAs per SM for the persistent grid (0 = auto);  */
                                     /* with PDM_PATH_CLUSTER: the cluster size 2, 4 or 8 (0 = auto) */
                                     /* with PDM_PATH_PACKED: depth steps per tile visit T (0 = auto) */
+                                    /* with PDM_PATH_TILED: depth steps per launch, 1 or 2 (0 = auto)*/
 #define PDM_PRESTACK      (1u << 21) /* plan for pdm_migrate_shot (shot-profile prestack migration,    */
                                     /* PAPER.md:151): always the PDM_PATH_PACKED form (AUTO or PACKED   */
                                     /* path bits), any table; pdm_migrate refuses such a plan           */

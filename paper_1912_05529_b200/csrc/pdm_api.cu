@@ -714,13 +714,43 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         }
         if (per_sm < 1) return PDM_ERR_UNSUPPORTED;
         p->ctas_per_sm = per_sm;
+        // Two depth steps per launch (pdm_tiled_step2) where the one-step kernel is HBM-bound: short
+        // filters (halo <= 2 groups) on warp-uniform models; bits 16-19 force 1 or 2 steps per launch
+        int xt = xtiles;
+        {
+            const unsigned tsel = (want == PDM_PATH_TILED) ? (p->flags >> PDM_CTAS_SHIFT) & 0xFu : 0u;
+            if (tsel > 2) return PDM_ERR_UNSUPPORTED;
+            const bool can2 = Lk <= 15 && nz >= 2;
+            if (tsel == 2 && !can2) return PDM_ERR_UNSUPPORTED;
+            // measured (layers, nx = 16384 / 32768): 15 taps 1.04-1.2x, 25 taps 0.92-0.95x -> AUTO only up to L = 7
+            if (can2 && (tsel == 2 || (tsel == 0 && !p->contiguous_rows && Lk <= 7))) {
+                const int keep = 32 - 2 * HG;
+                p->tile_x2 = (PDM_TILED_THREADS / 32) * keep * R;
+                p->smem_bytes2 = (PDM_TILED_THREADS / 32) * ((PDM_TILED_STAGES + 1) * (32 + 2 * HG) + 32) * (R + 2) * (int)sizeof(float2);
+                int per_sm2 = 0;
+                for (int wide = 0; wide < 2; ++wide) {
+                    tiled_fn fn2 = pdm_tiled2_kernel_for(Lk, wide != 0, p->sym != 0);
+                    if (!fn2) return PDM_ERR_UNSUPPORTED;
+                    PDM_CUDA(p, cudaFuncSetAttribute((const void *)fn2, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                     p->smem_bytes2));
+                    PDM_CUDA(p, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm2, (const void *)fn2,
+                                                                              PDM_TILED_THREADS, (size_t)p->smem_bytes2));
+                }
+                if (per_sm2 >= 1) {
+                    p->tiled_T2 = 1;
+                    per_sm = per_sm2;
+                    p->ctas_per_sm = per_sm2;
+                    xt = (nx + p->tile_x2 - 1) / p->tile_x2;
+                }
+            }
+        }
         // ONE resident wave per depth step: x-tiles x frequency groups <= SMs x CTAs per SM
-        int wgroups = std::max(1, std::min(nw, p->sm_count * per_sm / xtiles));
+        int wgroups = std::max(1, std::min(nw, p->sm_count * per_sm / xt));
         const int wpg = (nw + wgroups - 1) / wgroups;
         wgroups = (nw + wpg - 1) / wpg;
         p->wgroups = wgroups;
-        p->grid = xtiles * wgroups;
-        p->launches = nz + 1;
+        p->grid = xt * wgroups;
+        p->launches = (p->tiled_T2 ? nz / 2 + (nz & 1) : nz) + 1;
         p->n_partial = wgroups;
         if ((rc = dev_upload(p, &p->d_half, half.data(), half.size())) != PDM_OK) return rc;
         if ((rc = dev_alloc(p, &p->d_partial, (size_t)wgroups * nz * p->qstride)) != PDM_OK) return rc;
@@ -831,6 +861,20 @@ static int migrate_impl(pdm_plan *p, const pdm_c64 *P0_dev, const pdm_c64 *src_d
         dim3 grid((nx + p->tile_x - 1) / p->tile_x, p->wgroups);
         const float2 *src = P0;
         if (p->profiling) PDM_CUDA(p, cudaEventRecord(p->ev[0], st));
+        if (p->tiled_T2) {                               // two depth steps per launch; an odd last step alone
+            tiled_fn fn2 = pdm_tiled2_kernel_for(Lk, wide, p->sym != 0);
+            dim3 grid2((nx + p->tile_x2 - 1) / p->tile_x2, p->wgroups);
+            int k = 0;
+            for (int z = 0; z + 1 < nz; z += 2, ++k) {
+                a.z = z; a.Pin = src; a.Pout = p->d_plane[k & 1];
+                fn2<<<grid2, PDM_TILED_THREADS, p->smem_bytes2, st>>>(a);
+                src = a.Pout;
+            }
+            if (nz & 1) {
+                a.z = nz - 1; a.Pin = src; a.Pout = p->d_plane[k & 1];
+                fn<<<grid, PDM_TILED_THREADS, p->smem_bytes, st>>>(a);
+            }
+        } else
         for (int z = 0; z < nz; ++z) {
             a.z = z; a.Pin = src; a.Pout = p->d_plane[z & 1];
             fn<<<grid, PDM_TILED_THREADS, p->smem_bytes, st>>>(a);

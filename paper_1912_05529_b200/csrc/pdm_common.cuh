@@ -55,6 +55,7 @@ struct pdm_plan {
     int R;                // outputs per thread of the register-tiled kernels
     int threads, grid, ctas_per_sm, smem_bytes, launches;
     int tile_x, wgroups;  // tiled path
+    int tiled_T2, tile_x2, smem_bytes2;   // tiled path: two depth steps per launch (pdm_tiled_step2), its x-tile and smem
     int cluster_size, cluster_gper, cluster_passes;   // cluster path: CTAs per line, groups per CTA, passes per step
     int taps_in_smem;     // march: 1 = per-omega rows staged in shared memory, 0 = L1/L2 global rows
     // packed path (kern_pack.cuh): planes [nw][nxp] ping-pong, T depth steps per tile visit

@@ -26,6 +26,7 @@ march_fn pdm_march_kernel_part1(int L, bool taps_smem, bool dedup, int R);
 march_fn pdm_march_kernel_part2(int L, bool taps_smem, bool dedup, int R);
 cluster_fn pdm_cluster_kernel_for(int L, bool taps_smem, bool dedup);
 tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias);
+tiled_fn pdm_tiled2_kernel_for(int L, bool wide, bool sym);   // two depth steps per launch, L <= 15
 
 // general (asymmetric-table) builds: R = PDM_R, no row de-duplication / texture share (tu_asym.cu,
 // compiled in the same three parts of the filter-length list)

@@ -11,3 +11,15 @@ tiled_fn pdm_tiled_kernel_for(int L, bool wide, bool alias)
     default: return nullptr;
     }
 }
+
+// two depth steps per launch: short filters only (halo of at most 2 groups per side)
+tiled_fn pdm_tiled2_kernel_for(int L, bool wide, bool sym)
+{
+    switch (L) {
+#define X(LL) case LL: return sym ? (wide ? pdm_tiled_step2<LL, PDM_R, 2, true> : pdm_tiled_step2<LL, PDM_R, 1, true>) \
+                                  : (wide ? pdm_tiled_step2<LL, PDM_R, 2, false> : pdm_tiled_step2<LL, PDM_R, 1, false>);
+        PDM_L_PART0(X) X(15)
+#undef X
+    default: return nullptr;
+    }
+}

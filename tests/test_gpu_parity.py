@@ -222,6 +222,30 @@ def test_packed_path_with_unaligned_p0_pointer(pdm):
     assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
 
 
+@pytest.mark.parametrize("steps", [1, 2])
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps,sym", [
+    ("layers", 2500, 31, 6, 15, True),     # odd nz: the last step runs alone; 2 x-tiles of 8 x 240 samples
+    ("field", 300, 8, 7, 25, True),        # halo of 2 groups: 28 of 32 groups kept; nx below one warp tile
+    ("white", 5000, 5, 3, 31, True),       # L = 15: the longest filter of the two-step kernel
+    ("const", 129, 12, 3, 7, False),       # general (asymmetric) table
+    ("layers", 1921, 6, 40, 3, True),      # odd nx: 8-byte copies; several frequency groups
+])
+def test_tiled_path_two_depth_steps_per_launch(pdm, steps, model, nx, nz, nw, ntaps, sym):
+    """SURVEY 8(f) N2 at warp granularity: pdm_tiled_step2 keeps a warp's sub-tile on chip for two depth
+    steps (planes cross HBM once per two steps); forced 1 and 2 steps per launch must both match the
+    oracle, and agree with each other bit for bit (same arithmetic, same summation order)."""
+    cfg = pdm_inputs.random_problem(41, nx, nz, nw, ntaps, model=model, symmetric=sym)
+    flags = pdm.PDM_PATH_TILED | (steps << pdm.PDM_CTAS_SHIFT)
+    img, info = gpu_migrate(pdm, cfg, flags, want_info=True)
+    assert info["path"] == pdm.PDM_PATH_TILED
+    assert info["launches_per_migrate"] == (nz if steps == 1 else nz // 2 + nz % 2) + 1
+    rel, mx = errors(img, oracle.migrate(cfg))
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info)
+    if steps == 2:
+        one = gpu_migrate(pdm, cfg, pdm.PDM_PATH_TILED | (1 << pdm.PDM_CTAS_SHIFT))
+        assert np.array_equal(one, img)
+
+
 @pytest.mark.parametrize("nx,nz,nw,ntaps,model,csize", [
     (1000, 24, 5, 25, "white", 4),       # 125 groups over 4 CTAs of one warp: ragged last CTA
     (129, 50, 3, 35, "const", 8),        # 17 groups over 8 CTAs: most CTAs of a cluster idle
