@@ -45,6 +45,12 @@ def _load():
         lib.pdm_oracle_index.argtypes = [ctypes.c_float, ctypes.c_float, ctypes.c_double,
                                          ctypes.c_double, ctypes.c_int]
         lib.pdm_oracle_num_threads.restype = ctypes.c_int
+        lib.pdm_oracle_migrate3d.restype = ctypes.c_int
+        lib.pdm_oracle_migrate3d.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         lib.pdm_oracle_migrate_shot.restype = ctypes.c_int
         lib.pdm_oracle_migrate_shot.argtypes = [
             ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
@@ -128,3 +134,25 @@ def migrate_shot(cfg: dict, S0, R0, image=None) -> np.ndarray:
     if rc != 0:
         raise RuntimeError(f"pdm_oracle_migrate_shot failed with code {rc}")
     return image
+
+
+def migrate3d(cfg: dict, want_field: bool = False):
+    """3-D variant (reading R18): cfg has nx, ny, nz, nw, dz, du, omega [nw], velocity [nz, ny, nx],
+    table [ntab, ntaps, ntaps] (ky slow, kx fast), P0 [nw, ny, nx].  -> image float64 [nz, ny, nx]
+    (and the final wavefield complex128 [nw, ny, nx] when want_field)."""
+    lib = _load()
+    nx, ny, nz, nw = cfg["nx"], cfg["ny"], cfg["nz"], cfg["nw"]
+    omega = np.ascontiguousarray(cfg["omega"], dtype=np.float32)
+    velocity = np.ascontiguousarray(cfg["velocity"], dtype=np.float32)
+    table = np.ascontiguousarray(cfg["table"], dtype=np.complex64)
+    P0 = np.ascontiguousarray(cfg["P0"], dtype=np.complex64)
+    ntab, ntaps, ntaps2 = table.shape
+    assert ntaps == ntaps2 and omega.shape == (nw,) and velocity.shape == (nz, ny, nx) and P0.shape == (nw, ny, nx)
+    image = np.zeros((nz, ny, nx), dtype=np.float64)
+    field = np.zeros((nw, ny, nx), dtype=np.complex128) if want_field else None
+    rc = lib.pdm_oracle_migrate3d(nx, ny, nz, nw, float(cfg["dz"]), omega.ctypes.data, velocity.ctypes.data,
+                                  table.ctypes.data, ntab, ntaps, float(cfg["du"]), P0.ctypes.data,
+                                  image.ctypes.data, None if field is None else field.ctypes.data)
+    if rc != 0:
+        raise RuntimeError(f"pdm_oracle_migrate3d failed with code {rc}")
+    return (image, field) if want_field else image

@@ -256,3 +256,103 @@ int pdm_oracle_migrate_shot(int nx, int nz, int nw, double dz,
     free(q32);
     return ORACLE_OK;
 }
+
+/*
+ * 3-D variant -- PAPER.md:41 ("can be easily extended to the 3-D depth migration, which requires
+ * 2-D filters as extrapolators"), :47.  The paper gives Eq. (1) for one lateral axis only; reading
+ * R18 of DESIGN.md writes it out for two:
+ *
+ *   T1  q32[z][y][x] = (float)(dz / (v32[z][y][x] * du))                          (R3 unchanged)
+ *   T2  per frequency and depth step, per OUTPUT point (y, x):
+ *         idx = clamp(lrintf(w32 * q32[z][y][x]), 0, ntab-1)
+ *         P'(y,x) = sum_{ky=-L..L} sum_{kx=-L..L} table[idx][L+ky][L+kx] * P(y-ky, x-kx),
+ *         terms outside the grid dropped (R5); the (ky, kx) orientation is Eq. (1)'s x_{i-n} on both axes
+ *   T3  image[z][y][x] = sum_w Re P'(y,x) after the step (R6, R10)
+ *
+ * table is [ntab][ntaps][ntaps] (ky slow, kx fast).  OpenMP over frequencies, per-thread FP64 image
+ * accumulators summed in thread order.  wavefield_out (optional): final field [nw][ny][nx] complex double.
+ * Pins (tests/test_oracle_3d_pins.py): delta table, brute force, 2-D spectral identity with an
+ * asymmetric table, separable table == two passes of the (pinned) 1-D oracle, x<->y transposition.
+ */
+int pdm_oracle_migrate3d(int nx, int ny, int nz, int nw, double dz,
+                         const float *omega, const float *velocity,
+                         const oracle_c64 *table, int ntab, int ntaps, double du,
+                         const oracle_c64 *P0, double *image_out, double *wavefield_out)
+{
+    if (nx <= 0 || ny <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0 ||
+        !(du > 0.0) || !omega || !velocity || !table || !P0 || !image_out)
+        return ORACLE_ERR_ARG;
+    const int L = (ntaps - 1) / 2;
+    const size_t slab = (size_t)ny * (size_t)nx, vol = (size_t)nz * slab;
+    float *q32 = (float *)malloc(vol * sizeof(float));
+    if (!q32) return ORACLE_ERR_NOMEM;
+    for (size_t i = 0; i < vol; ++i) q32[i] = oracle_q32(dz, velocity[i], du);      /* T1 */
+    int nthreads = pdm_oracle_num_threads();
+    if (nthreads > nw) nthreads = nw;
+    double *acc = (double *)calloc((size_t)nthreads * vol, sizeof(double));
+    if (!acc) { free(q32); return ORACLE_ERR_NOMEM; }
+    int failed = 0;
+#pragma omp parallel num_threads(nthreads)
+    {
+#ifdef _OPENMP
+        const int tid = omp_get_thread_num();
+#else
+        const int tid = 0;
+#endif
+        double *img = acc + (size_t)tid * vol;
+        double *P = (double *)malloc(sizeof(double) * 2 * slab);
+        double *Pn = (double *)malloc(sizeof(double) * 2 * slab);
+        if (!P || !Pn) {
+#pragma omp atomic write
+            failed = 1;
+        } else {
+#pragma omp for schedule(static)
+            for (int iw = 0; iw < nw; ++iw) {
+                const float w32 = omega[iw];
+                for (size_t i = 0; i < slab; ++i) {
+                    P[2 * i] = (double)P0[(size_t)iw * slab + i].re;
+                    P[2 * i + 1] = (double)P0[(size_t)iw * slab + i].im;
+                }
+                for (int z = 0; z < nz; ++z) {
+                    const float *qz = q32 + (size_t)z * slab;
+                    for (int y = 0; y < ny; ++y)
+                        for (int x = 0; x < nx; ++x) {                               /* T2 */
+                            const int j = oracle_idx(w32, qz[(size_t)y * nx + x], ntab);
+                            const oracle_c64 *row = table + (size_t)j * ntaps * ntaps;
+                            double ar = 0.0, ai = 0.0;
+                            for (int ky = -L; ky <= L; ++ky) {
+                                const int ys = y - ky;
+                                if (ys < 0 || ys >= ny) continue;
+                                for (int kx = -L; kx <= L; ++kx) {
+                                    const int xs = x - kx;
+                                    if (xs < 0 || xs >= nx) continue;
+                                    const oracle_c64 wv = row[(size_t)(L + ky) * ntaps + (L + kx)];
+                                    const double pr = P[2 * ((size_t)ys * nx + xs)], pi = P[2 * ((size_t)ys * nx + xs) + 1];
+                                    ar += (double)wv.re * pr - (double)wv.im * pi;
+                                    ai += (double)wv.re * pi + (double)wv.im * pr;
+                                }
+                            }
+                            Pn[2 * ((size_t)y * nx + x)] = ar;
+                            Pn[2 * ((size_t)y * nx + x) + 1] = ai;
+                        }
+                    { double *t = P; P = Pn; Pn = t; }
+                    double *islab = img + (size_t)z * slab;                          /* T3 */
+                    for (size_t i = 0; i < slab; ++i) islab[i] += P[2 * i];
+                }
+                if (wavefield_out)
+                    memcpy(wavefield_out + 2 * (size_t)iw * slab, P, sizeof(double) * 2 * slab);
+            }
+        }
+        free(P);
+        free(Pn);
+    }
+    if (!failed)
+        for (size_t i = 0; i < vol; ++i) {
+            double s = 0.0;
+            for (int t = 0; t < nthreads; ++t) s += acc[(size_t)t * vol + i];
+            image_out[i] = s;
+        }
+    free(acc);
+    free(q32);
+    return failed ? ORACLE_ERR_NOMEM : ORACLE_OK;
+}
