@@ -268,6 +268,35 @@ typedef struct {
 int pdm_design_table(pdm_c64 *table_host, int ntab, int ntaps, double tab_du, double dz_over_dx,
                      const pdm_design_opts *opts, void *cuda_stream);
 
+/*
+ * ---- 3-D variant ---------------------------------------------------------
+ * PAPER.md:41 ("the explicit f-x migration can be easily extended to the 3-D depth migration, which
+ * requires 2-D filters as extrapolators"), :47.  Eq. (1) on two lateral axes (reading R18):
+ *
+ *     P(z+dz, w, y, x) = sum_{ky=-L..L} sum_{kx=-L..L} W_{ky,kx}(u(x,y,z)) * P(z, w, y-ky, x-kx)
+ *     image[z][y][x]   = sum_w Re P(z+dz, w, y, x)
+ *
+ * with the same index rule (R3, from velocity[z][y][x]), zero terms outside the grid on both axes (R5)
+ * and rows as in R6/R7.  The table is general: no symmetry is assumed or needed.
+ *
+ * pdm3_create  -- omega HOST float[nw]; velocity HOST float[nz][ny][nx]; table HOST
+ *                 pdm_c64[ntab][ntaps][ntaps], table[j][L+ky][L+kx] = W_{ky,kx}(u_j), u_j = j*tab_du;
+ *                 flags: 0 or PDM_FORCE_GENERAL.  Errors as pdm_create; PDM_ERR_UNSUPPORTED for
+ *                 ntaps > 15 (the longest unrolled 2-D kernel; shorter odd lengths run on the next
+ *                 longer one with zero taps appended).
+ * pdm3_migrate -- P0_dev DEVICE pdm_c64[nw][ny][nx] (read-only), image_dev DEVICE float[nz][ny][nx]
+ *                 (overwritten).  Enqueue only (nz + 1 launches), deterministic.
+ * pdm3_get_info / pdm3_destroy -- as the 2-D calls (info.path reports 6; info.samples = nx*ny*nz*nw,
+ *                 counted_flops = 8*ntaps^2 per sample).
+ */
+typedef struct pdm3_plan pdm3_plan;
+int pdm3_create(pdm3_plan **out, int nx, int ny, int nz, int nw, float dz,
+                const float *omega, const float *velocity,
+                const pdm_c64 *table, int ntab, int ntaps, double tab_du, unsigned flags);
+int pdm3_migrate(pdm3_plan *plan, const pdm_c64 *P0_dev, float *image_dev, void *cuda_stream);
+int pdm3_get_info(const pdm3_plan *plan, pdm_info *out);
+int pdm3_destroy(pdm3_plan *plan);
+
 #ifdef __cplusplus
 }
 #endif

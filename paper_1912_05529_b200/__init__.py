@@ -4,7 +4,7 @@ Thin Python binding over the C-ABI library libpdm.so (include/pdm.h).  Argument 
 only: every step of the path (table look-up, FIR extrapolation, depth marching, imaging) runs
 in the CUDA kernels under csrc/.  PyTorch is used for device memory and streams.
 """
-from .binding import (Plan, SectionTransform, pdm_tf_create, pdm_tf_forward, pdm_tf_destroy, PdmError, load_library, pdm_create, pdm_migrate, pdm_migrate_host, pdm_migrate_shot,  # noqa: F401
+from .binding import (Plan, Plan3D, pdm3_create, SectionTransform, pdm_tf_create, pdm_tf_forward, pdm_tf_destroy, PdmError, load_library, pdm_create, pdm_migrate, pdm_migrate_host, pdm_migrate_shot,  # noqa: F401
                       pdm_destroy, pdm_get_info, pdm_strerror, pdm_debug_table_index,
                       pdm_fp32_peak, pdm_design_table, pdm_profile_enable, pdm_profile_read, PdmInfo, EXPORTED_SYMBOLS,
                       PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER, PDM_PATH_PACKED,

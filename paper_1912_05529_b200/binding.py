@@ -30,7 +30,8 @@ PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_migrate_shot", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
                     "pdm_profile_enable", "pdm_profile_read",
-                    "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy", "pdm_design_table")
+                    "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy", "pdm_design_table",
+                    "pdm3_create", "pdm3_migrate", "pdm3_get_info", "pdm3_destroy")
 
 
 class PdmInfo(ctypes.Structure):
@@ -99,6 +100,14 @@ def load_library(path: str | None = None):
     lib.pdm_tf_forward.argtypes = [vp, vp, vp, vp]
     lib.pdm_tf_destroy.restype = ci
     lib.pdm_tf_destroy.argtypes = [vp]
+    lib.pdm3_create.restype = ci
+    lib.pdm3_create.argtypes = [ctypes.POINTER(vp), ci, ci, ci, ci, cf, vp, vp, vp, ci, ci, cd, cu]
+    lib.pdm3_migrate.restype = ci
+    lib.pdm3_migrate.argtypes = [vp, vp, vp, vp]
+    lib.pdm3_get_info.restype = ci
+    lib.pdm3_get_info.argtypes = [vp, ctypes.POINTER(PdmInfo)]
+    lib.pdm3_destroy.restype = ci
+    lib.pdm3_destroy.argtypes = [vp]
     lib.pdm_design_table.restype = ci
     lib.pdm_design_table.argtypes = [vp, ci, ci, cd, cd, ctypes.POINTER(PdmDesignOpts), vp]
     _lib = lib
@@ -374,6 +383,81 @@ class Plan:
     def close(self):
         if self._h is not None:
             pdm_destroy(self._h)
+            self._h = None
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+# ------------------------------------------------------------------ 3-D variant
+def pdm3_create(nx, ny, nz, nw, dz, omega, velocity, table, tab_du, flags=0):
+    """-> (status, plan handle or None).  velocity [nz, ny, nx], table [ntab, ntaps, ntaps] HOST arrays."""
+    lib = load_library()
+    omega = np.ascontiguousarray(omega, dtype=np.float32)
+    velocity = np.ascontiguousarray(velocity, dtype=np.float32)
+    table = np.ascontiguousarray(table, dtype=np.complex64)
+    if omega.shape != (nw,) or velocity.shape != (nz, ny, nx) or table.ndim != 3 or table.shape[1] != table.shape[2]:
+        return PDM_ERR_INVALID_ARG, None
+    h = ctypes.c_void_p()
+    rc = lib.pdm3_create(ctypes.byref(h), int(nx), int(ny), int(nz), int(nw), float(dz), omega.ctypes.data,
+                         velocity.ctypes.data, table.ctypes.data, int(table.shape[0]), int(table.shape[1]),
+                         float(tab_du), int(flags))
+    return int(rc), (h if rc == PDM_OK else None)
+
+
+class Plan3D:
+    """Owns a pdm3_plan (3-D variant: 2-D extrapolators)."""
+
+    def __init__(self, nx, ny, nz, nw, dz, omega, velocity, table, tab_du, flags=0):
+        rc, handle = pdm3_create(nx, ny, nz, nw, dz, omega, velocity, table, tab_du, flags)
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm3_create")
+        self._h = handle
+        self.nx, self.ny, self.nz, self.nw = int(nx), int(ny), int(nz), int(nw)
+
+    @classmethod
+    def from_config(cls, cfg: dict, flags: int = 0) -> "Plan3D":
+        return cls(cfg["nx"], cfg["ny"], cfg["nz"], cfg["nw"], cfg["dz"], cfg["omega"], cfg["velocity"],
+                   cfg["table"], cfg["du"], flags)
+
+    @property
+    def info(self) -> dict:
+        out = PdmInfo()
+        rc = load_library().pdm3_get_info(self._h, ctypes.byref(out))
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm3_get_info")
+        return out.as_dict()
+
+    def migrate(self, P0, image=None, stream=None):
+        """P0: torch.complex64 CUDA [nw, ny, nx] -> image torch.float32 CUDA [nz, ny, nx] (async)."""
+        import torch
+        if not (P0.is_cuda and P0.dtype == torch.complex64 and P0.is_contiguous()
+                and tuple(P0.shape) == (self.nw, self.ny, self.nx)):
+            raise ValueError("P0 must be a contiguous CUDA complex64 tensor [nw, ny, nx]")
+        if image is None:
+            image = torch.empty((self.nz, self.ny, self.nx), dtype=torch.float32, device=P0.device)
+        elif not (image.is_cuda and image.dtype == torch.float32 and image.is_contiguous()
+                  and tuple(image.shape) == (self.nz, self.ny, self.nx)):
+            raise ValueError("image must be a contiguous CUDA float32 tensor [nz, ny, nx]")
+        st = (stream or torch.cuda.current_stream(P0.device)).cuda_stream
+        rc = load_library().pdm3_migrate(self._h, ctypes.c_void_p(P0.data_ptr()), ctypes.c_void_p(image.data_ptr()),
+                                         ctypes.c_void_p(st))
+        if rc != PDM_OK:
+            raise PdmError(rc, "pdm3_migrate")
+        return image
+
+    def close(self):
+        if getattr(self, "_h", None) is not None:
+            load_library().pdm3_destroy(self._h)
             self._h = None
 
     def __enter__(self):

@@ -17,6 +17,7 @@ OBJDIR = os.path.join(_HERE, "build")
 # (source, extra defines, object name)
 UNITS = [("pdm_api.cu", [], "pdm_api.o"),
          ("pdm_design.cu", [], "pdm_design.o"),
+         ("pdm3_api.cu", [], "pdm3_api.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=0"], "tu_march0.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=1"], "tu_march1.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=2"], "tu_march2.o"),
@@ -29,7 +30,7 @@ UNITS = [("pdm_api.cu", [], "pdm_api.o"),
          ("tu_cluster.cu", [], "tu_cluster.o"),
          ("tu_tiled.cu", [], "tu_tiled.o")]
 HEADERS = ["pdm_common.cuh", "pdm_dispatch.cuh", "kern_naive.cuh", "kern_peak.cuh", "kern_march.cuh",
-           "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh", "kern_reduce.cuh", "kern_pack.cuh", "kern_fft.cuh"]
+           "kern_tiled.cuh", "kern_tf.cuh", "kern_cluster.cuh", "kern_reduce.cuh", "kern_pack.cuh", "kern_fft.cuh", "kern_3d.cuh"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC"]
 

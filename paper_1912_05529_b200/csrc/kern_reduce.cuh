@@ -3,7 +3,7 @@
 #include "pdm_common.cuh"
 
 // A5, second half: image[z][x] = sum over CTAs (fixed order) of their partial images.
-__global__ void pdm_reduce_partials(const float *__restrict__ partial, float *__restrict__ image,
+static __global__ void pdm_reduce_partials(const float *__restrict__ partial, float *__restrict__ image,
                                     int nparts, int nz, int nx, int pstride)
 {
     const int x = blockIdx.x * blockDim.x + threadIdx.x;

@@ -432,3 +432,36 @@ def random_problem(seed: int, nx: int, nz: int, nw: int, ntaps: int, ntab: int =
     return dict(name=f"random {model} {nx}x{nz}x{nw} taps={ntaps}", nx=nx, nz=nz, nw=nw,
                 ntaps=ntaps, ntab=ntab, dx=dx, dz=dz, du=float(du), omega=omega,
                 velocity=np.ascontiguousarray(v_in), table=np.ascontiguousarray(table), P0=P0)
+
+
+def random_problem_3d(seed: int, nx: int, ny: int, nz: int, nw: int, ntaps: int, ntab: int = 64,
+                      model: str = "field"):
+    """Seeded 3-D problem: velocity [nz, ny, nx] ('const' | 'layers' | 'field' = smooth in
+    x, varying with y and z | 'white'), a random GENERAL 2-D table [ntab, ntaps, ntaps] scaled so that
+    sum |W| < 1 (stable for any index pattern), Gaussian P0 [nw, ny, nx]."""
+    rng = np.random.default_rng([seed, nx, ny, nz, nw, ntaps])
+    dz = 10.0
+    if model == "const":
+        v = np.full((nz, ny, nx), 2000.0)
+    elif model == "layers":
+        v = np.repeat(np.linspace(1500.0, 4500.0, nz)[:, None, None], ny, 1).repeat(nx, 2)
+    elif model == "field":
+        xs = np.linspace(0, 3.0, nx)[None, None, :]
+        ys = np.linspace(0, 2.0, ny)[None, :, None]
+        zs = np.linspace(0, 1.0, nz)[:, None, None]
+        v = np.clip(2500.0 + 900.0 * np.sin(2.1 * xs + 1.3 * ys) * np.cos(1.7 * ys + zs) + 800.0 * zs, 1500.0, 5000.0)
+    elif model == "white":
+        v = rng.uniform(1500.0, 5000.0, (nz, ny, nx))
+    else:
+        raise ValueError(model)
+    v_in = (0.5 * v).astype(np.float32)
+    omega = (2.0 * np.pi * np.linspace(3.0, 60.0, nw)).astype(np.float32)
+    du = _table_du(omega, dz, v_in, ntab)
+    table = (rng.standard_normal((ntab, ntaps, ntaps)) + 1j * rng.standard_normal((ntab, ntaps, ntaps)))
+    table = (table / (np.abs(table).sum(axis=(1, 2), keepdims=True) * 1.02)).astype(np.complex64)
+    P0 = np.empty((nw, ny, nx), dtype=np.complex64)
+    P0.real = rng.standard_normal((nw, ny, nx), dtype=np.float32)
+    P0.imag = rng.standard_normal((nw, ny, nx), dtype=np.float32)
+    return dict(name=f"random3d {model} {nx}x{ny}x{nz}x{nw} taps={ntaps}x{ntaps}", nx=nx, ny=ny, nz=nz, nw=nw,
+                ntaps=ntaps, ntab=ntab, dx=10.0, dy=10.0, dz=dz, du=float(du), omega=omega,
+                velocity=np.ascontiguousarray(v_in), table=np.ascontiguousarray(table), P0=P0)

@@ -22,7 +22,7 @@ def lib():
 def _declared_functions():
     text = open(os.path.join(ROOT, "include", "pdm.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(pdm_[a-z0-9_]+)\s*\(", text)))
+    return sorted(set(re.findall(r"\b(pdm3?_[a-z0-9_]+)\s*\(", text)))
 
 
 def test_header_declares_the_boundary():

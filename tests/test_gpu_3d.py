@@ -1,0 +1,76 @@
+"""GPU parity of the 3-D variant (pdm3_create / pdm3_migrate; PAPER.md:41, :47;
+reading R18) against pdm_oracle_migrate3d, element by element, at the north_star bar."""
+import numpy as np
+import pytest
+
+import oracle
+import pdm_inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def pdm():
+    import torch
+    import paper_1912_05529_b200 as m
+    assert torch.cuda.is_available(), "gpu tests need a B200"
+    m.load_library()
+    return m
+
+
+def _errors(got, ref):
+    d = got.astype(np.float64) - ref
+    return np.linalg.norm(d) / np.linalg.norm(ref), np.abs(d).max() / np.abs(ref).max()
+
+
+@pytest.mark.parametrize("model,nx,ny,nz,nw,ntaps", [
+    ("field", 70, 19, 5, 3, 3),        # one ragged tile; every sample its own row
+    ("white", 300, 20, 4, 5, 7),       # two x-tiles, three y-tiles; 7 x 7 operator
+    ("layers", 513, 9, 6, 4, 5),       # odd nx: 8-byte copies; warp-uniform rows
+    ("const", 64, 64, 3, 2, 15),       # the longest unrolled operator (15 x 15)
+    ("field", 260, 33, 3, 9, 9),       # 9 x 9 runs on the 11 x 11 kernel with zero taps appended; several w groups
+    ("field", 1, 1, 4, 2, 3),          # a single trace
+])
+def test_3d_matches_oracle(pdm, model, nx, ny, nz, nw, ntaps):
+    import torch
+    cfg = pdm_inputs.random_problem_3d(7, nx, ny, nz, nw, ntaps, model=model)
+    ref = oracle.migrate3d(cfg)
+    with pdm.Plan3D.from_config(cfg) as plan:
+        info = plan.info
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        a = plan.migrate(p0).clone()
+        b = plan.migrate(p0).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    rel, mx = _errors(a.cpu().numpy(), ref)
+    assert np.isfinite(a.cpu().numpy()).all() and rel <= 1e-4 and mx <= 1e-3, (rel, mx, info)
+
+
+def test_3d_force_general_and_unaligned_input(pdm):
+    import torch
+    cfg = pdm_inputs.random_problem_3d(9, 200, 12, 4, 3, 5, model="layers")
+    ref = oracle.migrate3d(cfg)
+    with pdm.Plan3D.from_config(cfg) as fast, pdm.Plan3D.from_config(cfg, pdm.PDM_FORCE_GENERAL) as gen:
+        p0 = torch.from_numpy(cfg["P0"]).cuda()
+        store = torch.empty(p0.numel() + 1, dtype=p0.dtype, device="cuda")
+        shifted = store[1:].view(p0.shape)
+        shifted.copy_(p0)
+        assert shifted.data_ptr() % 16 == 8
+        a = fast.migrate(p0).clone()
+        b = gen.migrate(p0).clone()
+        c = fast.migrate(shifted).clone()
+        torch.cuda.synchronize()
+    assert torch.equal(a, b) and torch.equal(a, c)
+    rel, mx = _errors(a.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx)
+
+
+def test_3d_error_codes(pdm):
+    cfg = pdm_inputs.random_problem_3d(3, 16, 8, 2, 2, 3)
+    args = (cfg["nx"], cfg["ny"], cfg["nz"], cfg["nw"], cfg["dz"], cfg["omega"], cfg["velocity"])
+    rc, h = pdm.pdm3_create(*args, np.zeros((4, 17, 17), np.complex64), cfg["du"])      # 17 x 17: no unrolled kernel
+    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
+    rc, h = pdm.pdm3_create(*args, cfg["table"][:, :2, :2], cfg["du"])                   # even ntaps
+    assert rc == pdm.PDM_ERR_INVALID_ARG and h is None
+    rc, h = pdm.pdm3_create(*args, cfg["table"], cfg["du"] * 0.5)                         # table too short
+    assert rc == pdm.PDM_ERR_TABLE_RANGE and h is None
