@@ -577,6 +577,53 @@ def run_prestack(args):
                       "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12)}), flush=True)
 
 
+# ------------------------------------------------------------------------------- 3-D variant
+def run_3d(args):
+    """the 3-D variant (2-D extrapolators) on seeded 256 x 256 x 64 volumes,
+    64 frequencies; one JSON line per (operator size, velocity model).  Counted flops: 8 x ntaps^2 per sample."""
+    import torch
+
+    import paper_1912_05529_b200 as pdm
+    import pdm_inputs
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback")
+    pdm.load_library()
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    stream = torch.cuda.current_stream(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    nx = ny = 256; nz = 64; nw = 64
+    for ntaps in (7, 15):
+        for model in ("layers", "field"):
+            cfg = pdm_inputs.random_problem_3d(5, nx, ny, nz, nw, ntaps, model=model)
+            P0 = torch.from_numpy(cfg["P0"]).to(dev)
+            image = torch.empty((nz, ny, nx), dtype=torch.float32, device=dev)
+            with pdm.Plan3D.from_config(cfg, args.flags) as plan:
+                info = plan.info
+                for _ in range(max(args.warmup, 3)):
+                    plan.migrate(P0, image, stream=stream)
+                torch.cuda.synchronize(dev)
+                ms = []
+                for _ in range(args.steps):
+                    flush.zero_()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream)
+                    plan.migrate(P0, image, stream=stream)
+                    b.record(stream)
+                    torch.cuda.synchronize(dev)
+                    ms.append(a.elapsed_time(b))
+            t = float(np.median(ms)) * 1e-3
+            sps = info["samples"] / t
+            hbm_gbs, _ = measured_hbm_gbs()
+            print(json.dumps({"workload": f"3-D nx={nx} ny={ny} nz={nz} nw={nw} taps={ntaps}x{ntaps} velocity={model}",
+                              "kernel": "pdm3_step", "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
+                              "smem_bytes": info["smem_bytes"], "steps": args.steps, "ms": t * 1e3,
+                              "ms_best": float(min(ms)), "samples_per_s": sps,
+                              "frac_fp32_peak_counted": sps * 8 * ntaps * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                              "frac_hbm_16B_per_sample": sps * 16 / (hbm_gbs * 1e9)}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -589,6 +636,7 @@ def main():
     ap.add_argument("--no-extra", action="store_true",
                     help="skip extra.other_configs (configs[0..2] + two configs[4] points, N = 1 only)")
     ap.add_argument("--tf", action="store_true", help="time the t->f transform of the section (SURVEY 8(f) N1)")
+    ap.add_argument("--3d", dest="three_d", action="store_true", help="time the 3-D variant (SURVEY 8(f) N4)")
     ap.add_argument("--prestack", action="store_true", help="time one prestack shot (SURVEY 8(f) N4)")
     ap.add_argument("--sweep", action="store_true", help="configs[4] throughput sweep, one JSON line per point")
     ap.add_argument("--sweep-taps", default="", help="comma list of tap counts to sweep (default 15,25,51)")
@@ -600,7 +648,7 @@ def main():
     args = ap.parse_args()
     if args.gpus < 1:
         raise SystemExit("bench.py: --gpus must be >= 1")
-    multi = not (args.tf or args.sweep or args.prestack)
+    multi = not (args.tf or args.sweep or args.prestack or args.three_d)
     if multi and args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # not under torchrun: start the N ranks ourselves (one process per GPU, NCCL), loudly
         # refusing a box with fewer GPUs -- never a silent 1-rank run that prints n_gpus: 1
@@ -624,6 +672,9 @@ def main():
     if args.tf:
         if rank == 0:
             run_tf(args)
+    elif args.three_d:
+        if rank == 0:
+            run_3d(args)
     elif args.prestack:
         if rank == 0:
             run_prestack(args)

@@ -31,6 +31,57 @@ struct pdm3_params {
     int force_general;
 };
 
+// One ky pass: acc += sum_kx W[ky][kx] * P(y-ky, x-kx) for the thread's 8 outputs -- the general
+// (unfolded) register-tiled FIR of kern_march.cuh, accumulating.  tb + toff[r] = first unit of this ky's
+// taps in the table row of output r (all equal when UNIFORM: one broadcast load per tap pair).
+template <int L, bool UNIFORM>
+__device__ __forceinline__ void pdm3_pass(const float2 *__restrict__ base, const float4 *__restrict__ tb,
+                                          const int (&toff)[8], float2 (&acc_a)[8], float2 (&acc_b)[8])
+{
+    constexpr int R = 8;
+    float2 wl[R], wr[R];
+    float4 tw[UNIFORM ? 1 : R];
+#pragma unroll
+    for (int i = 0; i < R / 2; ++i) {
+        const float4 v = *reinterpret_cast<const float4 *>(base + 2 * i);
+        wl[2 * i] = f4lo(v); wl[2 * i + 1] = f4hi(v);
+        wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
+    }
+#pragma unroll
+    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = __ldg(tb + toff[r]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {                          // kx = 0
+        const float4 t = tw[UNIFORM ? 0 : r];
+        acc_a[r] = pk_fma_s(wl[r].x, f4lo(t), acc_a[r]);
+        acc_b[r] = pk_fma_s(wl[r].y, f4lo(t), acc_b[r]);
+    }
+    float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
+#pragma unroll
+    for (int k = 1; k <= L; ++k) {
+        if (k & 1) {
+            lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(-k - 1));
+            rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(R + k - 1));
+            wl[pdm_mod(-k, R)] = f4hi(lv);
+            wr[pdm_mod(k - 1, R)] = f4lo(rv);
+        } else {
+            wl[pdm_mod(-k, R)] = f4lo(lv);
+            wr[pdm_mod(k - 1, R)] = f4hi(rv);
+        }
+#pragma unroll
+        for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = __ldg(tb + toff[r] + k);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            const float2 a = wl[pdm_mod(r - k, R)];         // P(y-ky, x-kx): times W[ky][kx]
+            const float2 b = wr[pdm_mod(r + k, R)];         // P(y-ky, x+kx): times W[ky][-kx]
+            acc_a[r] = pk_fma_s(a.x, f4lo(t), acc_a[r]);
+            acc_b[r] = pk_fma_s(a.y, f4lo(t), acc_b[r]);
+            acc_a[r] = pk_fma_s(b.x, f4hi(t), acc_a[r]);
+            acc_b[r] = pk_fma_s(b.y, f4hi(t), acc_b[r]);
+        }
+    }
+}
+
 template <int L, int CH>
 __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p)
 {
@@ -99,61 +150,17 @@ __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p
 #pragma unroll
         for (int r = 0; r < R; ++r) { acc_a[r] = make_float2(0.f, 0.f); acc_b[r] = make_float2(0.f, 0.f); }
 
-#pragma unroll 1
-        for (int ky = -L; ky <= L; ++ky) {                 // one 1-D pass per ky: row y-ky, taps W[ky][.]
-            const float2 *base = tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS;
-            const float4 *tb = p.tab + (ky + L) * (L + 1);
-            float2 wl[R], wr[R];
-            float4 tw[R];
-#pragma unroll
-            for (int i = 0; i < R / 2; ++i) {
-                const float4 v = *reinterpret_cast<const float4 *>(base + 2 * i);
-                wl[2 * i] = f4lo(v); wl[2 * i + 1] = f4hi(v);
-                wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
-            }
-            if (uni) {
-                const float4 t = __ldg(tb + toff[0]);
-#pragma unroll
-                for (int r = 0; r < R; ++r) tw[r] = t;
-            } else {
-#pragma unroll
-                for (int r = 0; r < R; ++r) tw[r] = __ldg(tb + toff[r]);
-            }
-#pragma unroll
-            for (int r = 0; r < R; ++r) {                  // kx = 0
-                acc_a[r] = pk_fma_s(wl[r].x, f4lo(tw[r]), acc_a[r]);
-                acc_b[r] = pk_fma_s(wl[r].y, f4lo(tw[r]), acc_b[r]);
-            }
-            float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
-#pragma unroll
-            for (int k = 1; k <= L; ++k) {
-                if (k & 1) {
-                    lv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(-k - 1));
-                    rv = *reinterpret_cast<const float4 *>(base + pdm_soff<R>(R + k - 1));
-                    wl[pdm_mod(-k, R)] = f4hi(lv);
-                    wr[pdm_mod(k - 1, R)] = f4lo(rv);
-                } else {
-                    wl[pdm_mod(-k, R)] = f4lo(lv);
-                    wr[pdm_mod(k - 1, R)] = f4hi(rv);
-                }
-                if (uni) {
-                    const float4 t = __ldg(tb + toff[0] + k);
-#pragma unroll
-                    for (int r = 0; r < R; ++r) tw[r] = t;
-                } else {
-#pragma unroll
-                    for (int r = 0; r < R; ++r) tw[r] = __ldg(tb + toff[r] + k);
-                }
-#pragma unroll
-                for (int r = 0; r < R; ++r) {
-                    const float2 a = wl[pdm_mod(r - k, R)];     // P(y-ky, x-kx): times W[ky][kx]
-                    const float2 b = wr[pdm_mod(r + k, R)];     // P(y-ky, x+kx): times W[ky][-kx]
-                    acc_a[r] = pk_fma_s(a.x, f4lo(tw[r]), acc_a[r]);
-                    acc_b[r] = pk_fma_s(a.y, f4lo(tw[r]), acc_b[r]);
-                    acc_a[r] = pk_fma_s(b.x, f4hi(tw[r]), acc_a[r]);
-                    acc_b[r] = pk_fma_s(b.y, f4hi(tw[r]), acc_b[r]);
-                }
-            }
+        // one 1-D pass per ky (row y-ky, taps W[ky][.]); short operators: all 2L+1 passes unrolled
+        if (uni) {
+#pragma unroll (L <= 3 ? 2 * L + 1 : 1)
+            for (int ky = -L; ky <= L; ++ky)
+                pdm3_pass<L, true>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,
+                                   p.tab + (ky + L) * (L + 1), toff, acc_a, acc_b);
+        } else {
+#pragma unroll (L <= 3 ? 2 * L + 1 : 1)
+            for (int ky = -L; ky <= L; ++ky)
+                pdm3_pass<L, false>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,
+                                    p.tab + (ky + L) * (L + 1), toff, acc_a, acc_b);
         }
         if (active) {
             float2 out[R];
