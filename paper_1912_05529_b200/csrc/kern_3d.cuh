@@ -29,12 +29,13 @@ struct pdm3_params {
     int qstride, pstride;
     int z, w_per_group;
     int force_general;
+    int slice_rows;          // table rows the shared-memory slice holds (0: rows are read through L1)
 };
 
 // One ky pass: acc += sum_kx W[ky][kx] * P(y-ky, x-kx) for the thread's 8 outputs -- the general
 // (unfolded) register-tiled FIR of kern_march.cuh, accumulating.  tb + toff[r] = first unit of this ky's
 // taps in the table row of output r (all equal when UNIFORM: one broadcast load per tap pair).
-template <int L, bool UNIFORM>
+template <int L, bool UNIFORM, bool STAGED = false>
 __device__ __forceinline__ void pdm3_pass(const float2 *__restrict__ base, const float4 *__restrict__ tb,
                                           const int (&toff)[8], float2 (&acc_a)[8], float2 (&acc_b)[8])
 {
@@ -48,7 +49,7 @@ __device__ __forceinline__ void pdm3_pass(const float2 *__restrict__ base, const
         wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
     }
 #pragma unroll
-    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = __ldg(tb + toff[r]);
+    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = STAGED ? tb[toff[r]] : __ldg(tb + toff[r]);
 #pragma unroll
     for (int r = 0; r < R; ++r) {                          // kx = 0
         const float4 t = tw[UNIFORM ? 0 : r];
@@ -68,7 +69,7 @@ __device__ __forceinline__ void pdm3_pass(const float2 *__restrict__ base, const
             wr[pdm_mod(k - 1, R)] = f4hi(rv);
         }
 #pragma unroll
-        for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = __ldg(tb + toff[r] + k);
+        for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = STAGED ? tb[toff[r] + k] : __ldg(tb + toff[r] + k);
 #pragma unroll
         for (int r = 0; r < R; ++r) {
             const float4 t = tw[UNIFORM ? 0 : r];
@@ -94,6 +95,12 @@ __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p
     constexpr int UNITS = (2 * L + 1) * (L + 1);                 // float4 units per table row
     extern __shared__ __align__(16) unsigned char pdm_smem[];
     float2 *bufs = reinterpret_cast<float2 *>(pdm_smem);         // [2][NROW][NGX][GS]
+    // plans whose model gives (nearly) every sample its own row: the rows this tile can touch at this
+    // depth and frequency, [idx(w, q_min), idx(w, q_max)] with q over the tile, are staged per frequency
+    // (odd row stride: consecutive rows in distinct bank groups); too many rows -> read through L1
+    constexpr int UNITS_P = UNITS | 1;
+    float4 *slice = reinterpret_cast<float4 *>(bufs + 2 * BUF_SLOTS);
+    __shared__ float qred[2][PDM3_THREADS / 32];
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int tx0 = blockIdx.x * PDM3_TX, ty0 = blockIdx.y * PDM3_TY;
@@ -130,6 +137,22 @@ __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p
 #pragma unroll
     for (int r = 0; r < R; ++r) img[r] = 0.f;
     const bool active = y < p.ny && x0 < p.nx;
+    float tq_min = 0.f, tq_max = 0.f;
+    if (p.slice_rows > 0) {                                // q extrema of the tile (block reduction, once)
+        float lo = qc[0], hi = qc[0];
+#pragma unroll
+        for (int r = 1; r < R; ++r) { lo = fminf(lo, qc[r]); hi = fmaxf(hi, qc[r]); }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            lo = fminf(lo, __shfl_xor_sync(0xffffffffu, lo, o));
+            hi = fmaxf(hi, __shfl_xor_sync(0xffffffffu, hi, o));
+        }
+        if (lane == 0) { qred[0][warp] = lo; qred[1][warp] = hi; }
+        __syncthreads();
+        tq_min = qred[0][0]; tq_max = qred[1][0];
+#pragma unroll
+        for (int i = 1; i < PDM3_THREADS / 32; ++i) { tq_min = fminf(tq_min, qred[0][i]); tq_max = fmaxf(tq_max, qred[1][i]); }
+    }
 
     for (int iw = w_begin, it = 0; iw < w_end; ++iw, ++it) {
         const float w = p.omega[iw];
@@ -137,31 +160,47 @@ __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p
         __syncthreads();                                   // tile iw complete; everyone is done with tile iw-1
         if (iw + 1 < w_end) issue_load(iw + 1, (it + 1) & 1);
 
-        int toff[R];
+        int jidx[R], toff[R];
         bool un = true;
 #pragma unroll
         for (int r = 0; r < R; ++r) {
-            toff[r] = pdm_index(w, qc[r], ntab_m1) * UNITS;
-            un = un && (toff[r] == toff[0]);
+            jidx[r] = pdm_index(w, qc[r], ntab_m1);
+            toff[r] = jidx[r] * UNITS;
+            un = un && (jidx[r] == jidx[0]);
         }
         const bool uni = __all_sync(0xffffffffu, un && !p.force_general);
+        bool staged = false;
+        if (p.slice_rows > 0) {                            // CTA-uniform decisions
+            const int jlo = pdm_index(w, tq_min, ntab_m1), jhi = pdm_index(w, tq_max, ntab_m1);
+            staged = jhi > jlo && jhi - jlo + 1 <= p.slice_rows;
+            if (staged) {
+                const int nrows = jhi - jlo + 1;
+                for (int e = tid; e < nrows * UNITS; e += PDM3_THREADS) {
+                    const int rr = e / UNITS, u = e - rr * UNITS;
+                    slice[rr * UNITS_P + u] = __ldg(p.tab + (size_t)(jlo + rr) * UNITS + u);
+                }
+#pragma unroll
+                for (int r = 0; r < R; ++r) toff[r] = (jidx[r] - jlo) * UNITS_P;
+            }
+            __syncthreads();                               // slice complete (or nobody staged: still uniform)
+        }
         const float2 *tile = bufs + (size_t)(it & 1) * BUF_SLOTS;
         float2 acc_a[R], acc_b[R];
 #pragma unroll
         for (int r = 0; r < R; ++r) { acc_a[r] = make_float2(0.f, 0.f); acc_b[r] = make_float2(0.f, 0.f); }
 
         // one 1-D pass per ky (row y-ky, taps W[ky][.]); short operators: all 2L+1 passes unrolled
-        if (uni) {
-#pragma unroll (L <= 3 ? 2 * L + 1 : 1)
-            for (int ky = -L; ky <= L; ++ky)
-                pdm3_pass<L, true>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,
-                                   p.tab + (ky + L) * (L + 1), toff, acc_a, acc_b);
+#define PDM3_PASSES(UNI, ST, TB)                                                                     \
+        _Pragma("unroll (L <= 3 ? 2 * L + 1 : 1)")                                                      \
+        for (int ky = -L; ky <= L; ++ky)                                                                \
+            pdm3_pass<L, UNI, ST>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,               \
+                                  (TB) + (ky + L) * (L + 1), toff, acc_a, acc_b);
+        if (staged) {
+            if (uni) { PDM3_PASSES(true, true, slice) } else { PDM3_PASSES(false, true, slice) }
         } else {
-#pragma unroll (L <= 3 ? 2 * L + 1 : 1)
-            for (int ky = -L; ky <= L; ++ky)
-                pdm3_pass<L, false>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,
-                                    p.tab + (ky + L) * (L + 1), toff, acc_a, acc_b);
+            if (uni) { PDM3_PASSES(true, false, p.tab) } else { PDM3_PASSES(false, false, p.tab) }
         }
+#undef PDM3_PASSES
         if (active) {
             float2 out[R];
 #pragma unroll

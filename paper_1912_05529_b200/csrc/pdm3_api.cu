@@ -19,7 +19,7 @@ struct pdm3_plan {
     float *d_omega, *d_q, *d_partial;
     float4 *d_tab;
     float2 *d_plane[2];
-    int qstride, wgroups, smem_bytes, ctas_per_sm, grid;
+    int qstride, wgroups, smem_bytes, ctas_per_sm, grid, slice_rows;
     double workspace_bytes;
 };
 
@@ -110,11 +110,13 @@ extern "C" int pdm3_create(pdm3_plan **out, int nx, int ny, int nz, int nw, floa
     p->qstride = (nx + 7) / 8 * 8;
     std::vector<float> q((size_t)nz * ny * p->qstride);
     float qmax = 0.f, wmax = 0.f;
+    size_t varied = 0;                                     // rows whose q changes along x: per-sample table rows
     for (size_t r = 0; r < (size_t)nz * ny; ++r) {
         float *row = q.data() + r * p->qstride;
         for (int x = 0; x < nx; ++x) {
             row[x] = (float)((double)dz / ((double)velocity[r * nx + x] * tab_du));
             qmax = std::max(qmax, row[x]);
+            if (x && row[x] != row[x - 1]) { ++varied; }
         }
         for (int x = nx; x < p->qstride; ++x) row[x] = row[nx - 1];
     }
@@ -141,6 +143,14 @@ extern "C" int pdm3_create(pdm3_plan **out, int nx, int ny, int nz, int nw, floa
     PDM3_TRY(pdm3_alloc(p, &p->d_tab, tab.size(), tab.data()));
     const int HG = (Lk + 1 + 7) / 8;
     p->smem_bytes = 2 * (PDM3_TY + 2 * Lk) * (PDM3_TX / 8 + 2 * HG) * 10 * (int)sizeof(float2);
+    // models where (nearly) every sample has its own row: a per-tile, per-frequency slice of the table in
+    // shared memory (32 KB, 64 KB for the long operators) instead of gathering rows through L1
+    if (varied * 4 > (size_t)nz * ny * nx) {
+        const int units_p = ((2 * Lk + 1) * (Lk + 1)) | 1;
+        const int slice_bytes = (Lk <= 3 ? 32 : 64) * 1024;
+        p->slice_rows = slice_bytes / (units_p * (int)sizeof(float4));
+        p->smem_bytes += p->slice_rows * units_p * (int)sizeof(float4);
+    }
     int per_sm = 0;
     for (int wide = 0; wide < 2; ++wide) {
         pdm3_fn fn = pdm3_kernel_for(Lk, wide != 0);
@@ -178,6 +188,7 @@ extern "C" int pdm3_migrate(pdm3_plan *p, const pdm_c64 *P0_dev, float *image_de
     a.qstride = p->qstride; a.pstride = p->qstride;
     a.w_per_group = (p->nw + p->wgroups - 1) / p->wgroups;
     a.force_general = (p->flags & PDM_FORCE_GENERAL) ? 1 : 0;
+    a.slice_rows = p->slice_rows;
     // 16-byte copies and stores need every plane row 16-byte aligned: nx even and an aligned P0
     const bool wide = (p->nx % 2 == 0) && (((uintptr_t)P0_dev & 15u) == 0);
     pdm3_fn fn = pdm3_kernel_for(p->Lk, wide);
