@@ -145,7 +145,9 @@ int pdm_migrate(pdm_plan *plan, const pdm_c64 *P0_dev, float *image_dev, void *c
  * device, runs pdm_migrate, copies the image back and synchronises the stream before returning.
  *   P0_host    HOST pdm_c64[nw][nx] (pinned memory makes the copies asynchronous and faster).
  *   image_host HOST float[nz][nx].
- * Uses staging buffers owned by the plan (allocated on first use: PDM_ERR_NOMEM possible).
+ * Uses staging buffers owned by the plan (allocated on first use: PDM_ERR_NOMEM possible) -- except on
+ * the main (SMEM-marching) form with BOTH buffers pinned: the kernels then read P0 and write the image
+ * through the host mapping, so the transfers overlap the computation (same bits either way).
  */
 int pdm_migrate_host(pdm_plan *plan, const pdm_c64 *P0_host, float *image_host, void *cuda_stream);
 

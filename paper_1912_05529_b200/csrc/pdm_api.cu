@@ -979,6 +979,20 @@ extern "C" int pdm_migrate_host(pdm_plan *p, const pdm_c64 *P0_host, float *imag
     if (!p || !P0_host || !image_host || p->prestack) return PDM_ERR_INVALID_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const size_t nP = (size_t)p->nw * p->nx, nI = (size_t)p->nz * p->nx;
+    // Main form with PINNED host buffers: the kernels read P0 and write the image straight through the
+    // host mapping (each byte crosses the link once either way, but inside the marching / reduction
+    // kernels, overlapped with their work, instead of in two serial copies around them)
+    if (p->path == PDM_PATH_SMEM) {
+        cudaPointerAttributes ai, ao;
+        if (cudaPointerGetAttributes(&ai, P0_host) == cudaSuccess && cudaPointerGetAttributes(&ao, image_host) == cudaSuccess &&
+            ai.type == cudaMemoryTypeHost && ao.type == cudaMemoryTypeHost && ai.devicePointer && ao.devicePointer) {
+            int rc = pdm_migrate(p, (const pdm_c64 *)ai.devicePointer, (float *)ao.devicePointer, cuda_stream);
+            if (rc != PDM_OK) return rc;
+            PDM_CUDA(p, cudaStreamSynchronize(st));
+            return PDM_OK;
+        }
+        cudaGetLastError();
+    }
     if (!p->d_stage_p0) {
         int rc;
         if ((rc = dev_alloc(p, &p->d_stage_p0, nP)) != PDM_OK) return rc;

@@ -635,6 +635,12 @@ def test_migrate_host_equals_device_call(pdm):
         assert np.array_equal(host, dev.cpu().numpy())
         host2 = plan.migrate_host(cfg["P0"])
         assert np.array_equal(host2, host)
+        # both buffers pinned: the main form reads P0 and writes the image through the host mapping
+        # (no staging copies); same bits
+        out = torch.empty((cfg["nz"], cfg["nx"]), dtype=torch.float32).pin_memory()
+        assert plan.info["path"] == pdm.PDM_PATH_SMEM
+        plan.migrate_host(pinned, out)
+        assert np.array_equal(out.numpy(), host)
 
 
 def test_gpu_index_rule_matches_oracle_bit_for_bit(pdm):
