@@ -400,7 +400,12 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                "gpu_launches": int(info["launches_per_migrate"]) * k,
                "clocks": clocks}
         if world == 1 and not args.no_extra:
-            out["extra"] = {"other_configs": other_configs(pdm, torch, dev, stream, flush)}
+            import copy
+            a2 = copy.copy(args)
+            a2.flags, a2.steps = 0, min(args.steps, 5)
+            out["extra"] = {"other_configs": other_configs(pdm, torch, dev, stream, flush),
+                            # the stages around / beyond the poststack hot path, same run
+                            "other_stages": measure_tf(a2) + measure_prestack(a2) + measure_3d(a2)}
         print(json.dumps(out), flush=True)
     plan.close()
     if world > 1:
@@ -484,7 +489,7 @@ def run_sweep(args):
 
 
 # ------------------------------------------------------------------------------- t -> f transform
-def run_tf(args):
+def measure_tf(args):
     """the time -> frequency transform of the input section at configs[3]'s size
     (nt = 4096 samples, nx = 6144 traces, the 803 bins of 2-100 Hz), one JSON line."""
     import torch
@@ -522,7 +527,7 @@ def run_tf(args):
     # the section in and the band's bins out once; the contraction form (other nt) is FP32-bound
     hbm_gbs, hbm_src = measured_hbm_gbs()
     algo_bytes = 4.0 * nt * nx + 8.0 * bins.size * nx
-    print(json.dumps({"workload": f"t->f transform nt={nt} nx={nx} nw={bins.size} (configs[3] record)",
+    return [({"workload": f"t->f transform nt={nt} nx={nx} nw={bins.size} (configs[3] record)",
                       "kernel": "pdm_fft_kernel", "steps": args.steps, "ms": t * 1e3, "ms_best": float(min(ms)),
                       "bin_trace_outputs_per_s": bins.size * nx / t,
                       "roofline": {"bound": "hbm", "achieved": algo_bytes / t / 1e9, "peak": hbm_gbs,
@@ -530,11 +535,11 @@ def run_tf(args):
                                    "peak_source": hbm_src, "algorithmic_bytes": algo_bytes,
                                    "algorithmic_bytes_are": "section in (4 B x nt x nx) + P0 out (8 B x nw x nx)"},
                       "contraction_equivalent_tflops": 4.0 * nt * bins.size * nx / t / 1e12,
-                      "share_of_migration": "compare ms with bench.py's ms_per_step on configs[3]"}), flush=True)
+                      "share_of_migration": "compare ms with bench.py's ms_per_step on configs[3]"})]
 
 
 # ------------------------------------------------------------------------------- prestack shot
-def run_prestack(args):
+def measure_prestack(args):
     """one prestack shot (pdm_migrate_shot) on a configs[4] field point -- both
     wavefields are extrapolated, so a shot counts 2 x nx x nz x nw extrapolated samples."""
     import torch
@@ -570,15 +575,15 @@ def run_prestack(args):
             ms.append(a.elapsed_time(b))
     t = float(np.median(ms)) * 1e-3
     sps = info["samples"] / t
-    print(json.dumps({"workload": f"prestack shot, configs[4] field nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} "
+    return [({"workload": f"prestack shot, configs[4] field nx={nx} nz={cfg['nz']} nw={nw} taps={ntaps} "
                                   "(2 wavefields per frequency)", "kernel": "pdm_pack_kernel (xcorr)",
                       "path": PATH_NAMES[info["path"]], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                       "steps": args.steps, "ms": t * 1e3, "ms_best": float(min(ms)), "samples_per_s": sps,
-                      "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12)}), flush=True)
+                      "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12)})]
 
 
 # ------------------------------------------------------------------------------- 3-D variant
-def run_3d(args):
+def measure_3d(args):
     """the 3-D variant (2-D extrapolators) on seeded 256 x 256 x 64 volumes,
     64 frequencies; one JSON line per (operator size, velocity model).  Counted flops: 8 x ntaps^2 per sample."""
     import torch
@@ -594,6 +599,7 @@ def run_3d(args):
     stream = torch.cuda.current_stream(dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     nx = ny = 256; nz = 64; nw = 64
+    rows = []
     for ntaps in (7, 15):
         for model in ("layers", "field"):
             cfg = pdm_inputs.random_problem_3d(5, nx, ny, nz, nw, ntaps, model=model)
@@ -616,12 +622,28 @@ def run_3d(args):
             t = float(np.median(ms)) * 1e-3
             sps = info["samples"] / t
             hbm_gbs, _ = measured_hbm_gbs()
-            print(json.dumps({"workload": f"3-D nx={nx} ny={ny} nz={nz} nw={nw} taps={ntaps}x{ntaps} velocity={model}",
+            rows.append(({"workload": f"3-D nx={nx} ny={ny} nz={nz} nw={nw} taps={ntaps}x{ntaps} velocity={model}",
                               "kernel": "pdm3_step", "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                               "smem_bytes": info["smem_bytes"], "steps": args.steps, "ms": t * 1e3,
                               "ms_best": float(min(ms)), "samples_per_s": sps,
                               "frac_fp32_peak_counted": sps * 8 * ntaps * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
-                              "frac_hbm_16B_per_sample": sps * 16 / (hbm_gbs * 1e9)}), flush=True)
+                              "frac_hbm_16B_per_sample": sps * 16 / (hbm_gbs * 1e9)}))
+    return rows
+
+
+def run_tf(args):
+    for row in measure_tf(args):
+        print(json.dumps(row), flush=True)
+
+
+def run_prestack(args):
+    for row in measure_prestack(args):
+        print(json.dumps(row), flush=True)
+
+
+def run_3d(args):
+    for row in measure_3d(args):
+        print(json.dumps(row), flush=True)
 
 
 def main():
