@@ -74,3 +74,18 @@ def test_3d_error_codes(pdm):
     assert rc == pdm.PDM_ERR_INVALID_ARG and h is None
     rc, h = pdm.pdm3_create(*args, cfg["table"], cfg["du"] * 0.5)                         # table too short
     assert rc == pdm.PDM_ERR_TABLE_RANGE and h is None
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("model,ntaps", [("layers", 7), ("field", 7), ("field", 15)])
+def test_3d_at_bench_tile_counts(pdm, model, ntaps):
+    """The `bench.py --3d` lateral size (256 x 256: 32 y-tiles, several frequency groups, the staged slice
+    for the field model) on a shortened depth / frequency range the oracle finishes in seconds."""
+    import torch
+    cfg = pdm_inputs.random_problem_3d(5, 256, 256, 6, 5, ntaps, model=model)
+    ref = oracle.migrate3d(cfg)
+    with pdm.Plan3D.from_config(cfg) as plan:
+        img = plan.migrate(torch.from_numpy(cfg["P0"]).cuda())
+        torch.cuda.synchronize()
+    rel, mx = _errors(img.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx)

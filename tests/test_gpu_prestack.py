@@ -87,3 +87,26 @@ def test_prestack_argument_errors(pdm):
         z = torch.zeros((4, 200), dtype=torch.complex64, device="cuda")
         img = torch.zeros((5, 200), dtype=torch.float32, device="cuda")
         assert pdm.pdm_migrate_shot(plan._h, z.data_ptr(), z.data_ptr(), img.data_ptr(), False, 0) == pdm.PDM_ERR_INVALID_ARG
+
+
+@pytest.mark.slow
+def test_shot_at_bench_size_sampled_frequencies(pdm):
+    """The `bench.py --prestack` configuration (configs[4] field, nx = 4096, nw = 1024, 25 taps, AUTO T and
+    CTA size): 16 sampled frequencies carry data (first / last, pack boundaries, CTA range boundaries), the
+    other lines are zero, so the oracle only has to march those."""
+    import torch
+    from pdm_inputs.configs import sweep_point
+    cfg = sweep_point(4096, 1024, 25)
+    nw, nx = cfg["nw"], cfg["nx"]
+    lines = sorted({0, 1, 7, 8, 9, 511, 512, 1015, 1016, 1023, 137, 138, 300, 666, 777, 901})
+    rng = np.random.default_rng(99)
+    S0 = np.zeros((nw, nx), np.complex64); R0 = np.zeros((nw, nx), np.complex64)
+    s, r = _fields(rng, len(lines), nx)
+    S0[lines] = s; R0[lines] = r
+    sub = dict(cfg, nw=len(lines), omega=cfg["omega"][lines])
+    ref = oracle.migrate_shot(sub, s, r)
+    with pdm.Plan.from_config(cfg, pdm.PDM_PRESTACK) as plan:
+        img = plan.migrate_shot(torch.from_numpy(S0).cuda(), torch.from_numpy(R0).cuda())
+        torch.cuda.synchronize()
+        rel, mx = _errors(img.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx)
