@@ -600,9 +600,10 @@ def measure_3d(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
     nx = ny = 256; nz = 64; nw = 64
     rows = []
-    for ntaps in (7, 15):
-        for model in ("layers", "field"):
-            cfg = pdm_inputs.random_problem_3d(5, nx, ny, nz, nw, ntaps, model=model)
+    for ntaps, model, sym in ((7, "layers", False), (7, "field", False), (15, "layers", False), (15, "field", False),
+                              (7, "layers", True), (15, "layers", True), (15, "field", True)):
+        if True:
+            cfg = pdm_inputs.random_problem_3d(5, nx, ny, nz, nw, ntaps, model=model, symmetric=sym)
             P0 = torch.from_numpy(cfg["P0"]).to(dev)
             image = torch.empty((nz, ny, nx), dtype=torch.float32, device=dev)
             with pdm.Plan3D.from_config(cfg, args.flags) as plan:
@@ -622,7 +623,8 @@ def measure_3d(args):
             t = float(np.median(ms)) * 1e-3
             sps = info["samples"] / t
             hbm_gbs, _ = measured_hbm_gbs()
-            rows.append(({"workload": f"3-D nx={nx} ny={ny} nz={nz} nw={nw} taps={ntaps}x{ntaps} velocity={model}",
+            rows.append(({"workload": f"3-D nx={nx} ny={ny} nz={nz} nw={nw} taps={ntaps}x{ntaps} velocity={model}"
+                                      + (" operator symmetric in kx, ky (folded kernels)" if sym else ""),
                               "kernel": "pdm3_step", "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                               "smem_bytes": info["smem_bytes"], "steps": args.steps, "ms": t * 1e3,
                               "ms_best": float(min(ms)), "samples_per_s": sps,

@@ -279,11 +279,14 @@ int pdm_design_table(pdm_c64 *table_host, int ntab, int ntaps, double tab_du, do
  *     image[z][y][x]   = sum_w Re P(z+dz, w, y, x)
  *
  * with the same index rule (R3, from velocity[z][y][x]), zero terms outside the grid on both axes (R5)
- * and rows as in R6/R7.  The table is general: no symmetry is assumed or needed.
+ * and rows as in R6/R7.  The table is general: no symmetry is assumed or needed; a table that is bitwise
+ * symmetric in kx AND in ky (circularly symmetric extrapolators) runs on folded kernels (L+1 passes over
+ * row sums, (L+1)(6L+4) lane-ops per sample instead of 4(2L+1)^2), info.table_symmetric reports which.
  *
  * pdm3_create  -- omega HOST float[nw]; velocity HOST float[nz][ny][nx]; table HOST
  *                 pdm_c64[ntab][ntaps][ntaps], table[j][L+ky][L+kx] = W_{ky,kx}(u_j), u_j = j*tab_du;
- *                 flags: 0 or PDM_FORCE_GENERAL.  Errors as pdm_create; PDM_ERR_UNSUPPORTED for
+ *                 flags: 0, PDM_FORCE_GENERAL, PDM_REQUIRE_SYMMETRIC (refuse a table that is not doubly
+ *                 symmetric: PDM_ERR_TABLE_ASYMMETRIC).  Errors as pdm_create; PDM_ERR_UNSUPPORTED for
  *                 ntaps > 15 (the longest unrolled 2-D kernel; shorter odd lengths run on the next
  *                 longer one with zero taps appended).
  * pdm3_migrate -- P0_dev DEVICE pdm_c64[nw][ny][nx] (read-only), image_dev DEVICE float[nz][ny][nx]

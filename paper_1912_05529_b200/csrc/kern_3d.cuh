@@ -24,7 +24,8 @@ struct pdm3_params {
     float        *partial;   // [wgroups][nz][ny][pstride]
     const float  *q;         // [nz][ny][qstride]
     const float  *omega;     // [nw]
-    const float4 *tab;       // [ntab][2L+1][L+1] units (W[ky][kx], W[ky][-kx])
+    const float4 *tab;       // general: [ntab][2L+1][L+1] units (W[ky][kx], W[ky][-kx]); SYM2: [ntab][L+1][(L+2)/2]
+                             // units (W[ky][2t], W[ky][2t+1]), ky >= 0
     int nx, ny, nz, nw, ntab;
     int qstride, pstride;
     int z, w_per_group;
@@ -83,7 +84,69 @@ __device__ __forceinline__ void pdm3_pass(const float2 *__restrict__ base, const
     }
 }
 
-template <int L, int CH>
+// The same pass for operators that are bitwise symmetric in kx AND in ky (W[ky][kx] = W[-ky][kx] =
+// W[ky][-kx]: circularly symmetric 2-D extrapolators): the rows y-ky and y+ky are added while their
+// windows are loaded (TWO_ROWS; ky = 0 has one row) and the x-sum is folded as in the 1-D kernels,
+//   acc += W[ky][0] S(x) + sum_{kx>=1} W[ky][kx] (S(x-kx) + S(x+kx)),   S = P(y-ky,.) + P(y+ky,.)
+// 1 FADD2 + 2 FFMA2 per tap pair instead of 4 FFMA2, and L+1 passes instead of 2L+1.  Table units:
+// (W[ky][2t], W[ky][2t+1]) pairs, t = 0..L/2, for ky = 0..L.
+template <int L, bool UNIFORM, bool STAGED, bool TWO_ROWS>
+__device__ __forceinline__ void pdm3_pass_sym(const float2 *__restrict__ base, const float2 *__restrict__ base2,
+                                              const float4 *__restrict__ tb, const int (&toff)[8],
+                                              float2 (&acc_a)[8], float2 (&acc_b)[8])
+{
+    constexpr int R = 8;
+    float2 wl[R], wr[R];
+    float4 tw[UNIFORM ? 1 : R];
+    auto ld = [&](int off) {
+        float4 v = *reinterpret_cast<const float4 *>(base + off);
+        if (TWO_ROWS) {
+            const float4 u = *reinterpret_cast<const float4 *>(base2 + off);
+            const float2 a = pk_add(f4lo(v), f4lo(u)), b = pk_add(f4hi(v), f4hi(u));
+            v = make_float4(a.x, a.y, b.x, b.y);
+        }
+        return v;
+    };
+#pragma unroll
+    for (int i = 0; i < R / 2; ++i) {
+        const float4 v = ld(2 * i);
+        wl[2 * i] = f4lo(v); wl[2 * i + 1] = f4hi(v);
+        wr[2 * i] = f4lo(v); wr[2 * i + 1] = f4hi(v);
+    }
+#pragma unroll
+    for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = STAGED ? tb[toff[r]] : __ldg(tb + toff[r]);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {                          // kx = 0
+        const float4 t = tw[UNIFORM ? 0 : r];
+        acc_a[r] = pk_fma_s(wl[r].x, f4lo(t), acc_a[r]);
+        acc_b[r] = pk_fma_s(wl[r].y, f4lo(t), acc_b[r]);
+    }
+    float4 lv = make_float4(0.f, 0.f, 0.f, 0.f), rv = lv;
+#pragma unroll
+    for (int k = 1; k <= L; ++k) {
+        if (k & 1) {
+            lv = ld(pdm_soff<R>(-k - 1));
+            rv = ld(pdm_soff<R>(R + k - 1));
+            wl[pdm_mod(-k, R)] = f4hi(lv);
+            wr[pdm_mod(k - 1, R)] = f4lo(rv);
+        } else {
+            wl[pdm_mod(-k, R)] = f4lo(lv);
+            wr[pdm_mod(k - 1, R)] = f4hi(rv);
+#pragma unroll
+            for (int r = 0; r < (UNIFORM ? 1 : R); ++r) tw[r] = STAGED ? tb[toff[r] + k / 2] : __ldg(tb + toff[r] + k / 2);
+        }
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float4 t = tw[UNIFORM ? 0 : r];
+            const float2 W = (k & 1) ? f4hi(t) : f4lo(t);
+            const float2 sm = pk_add(wl[pdm_mod(r - k, R)], wr[pdm_mod(r + k, R)]);
+            acc_a[r] = pk_fma_s(sm.x, W, acc_a[r]);
+            acc_b[r] = pk_fma_s(sm.y, W, acc_b[r]);
+        }
+    }
+}
+
+template <int L, int CH, bool SYM2 = false>
 __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p)
 {
     constexpr int R = 8, GS = R + 2;
@@ -92,7 +155,8 @@ __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p
     constexpr int NROW = PDM3_TY + 2 * L;                        // tile rows incl. halo
     constexpr int ROW_SLOTS = NGX * GS;
     constexpr int BUF_SLOTS = NROW * ROW_SLOTS;
-    constexpr int UNITS = (2 * L + 1) * (L + 1);                 // float4 units per table row
+    constexpr int KU = SYM2 ? (L + 2) / 2 : L + 1;                // float4 units per ky
+    constexpr int UNITS = (SYM2 ? L + 1 : 2 * L + 1) * KU;       // float4 units per table row
     extern __shared__ __align__(16) unsigned char pdm_smem[];
     float2 *bufs = reinterpret_cast<float2 *>(pdm_smem);         // [2][NROW][NGX][GS]
     // plans whose model gives (nearly) every sample its own row: the rows this tile can touch at this
@@ -191,10 +255,20 @@ __global__ void __launch_bounds__(PDM3_THREADS, 2) pdm3_step(const pdm3_params p
 
         // one 1-D pass per ky (row y-ky, taps W[ky][.]); short operators: all 2L+1 passes unrolled
 #define PDM3_PASSES(UNI, ST, TB)                                                                     \
-        _Pragma("unroll (L <= 3 ? 2 * L + 1 : 1)")                                                      \
-        for (int ky = -L; ky <= L; ++ky)                                                                \
-            pdm3_pass<L, UNI, ST>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,               \
-                                  (TB) + (ky + L) * (L + 1), toff, acc_a, acc_b);
+        if (SYM2) {                                                                                     \
+            pdm3_pass_sym<L, UNI, ST, false>(tile + (warp + L) * ROW_SLOTS + (HG + lane) * GS, nullptr, \
+                                             (TB), toff, acc_a, acc_b);                                 \
+            _Pragma("unroll (L <= 3 ? L : 1)")                                                          \
+            for (int ky = 1; ky <= L; ++ky)                                                             \
+                pdm3_pass_sym<L, UNI, ST, true>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,  \
+                                                tile + (warp + L + ky) * ROW_SLOTS + (HG + lane) * GS,  \
+                                                (TB) + ky * KU, toff, acc_a, acc_b);                    \
+        } else {                                                                                        \
+            _Pragma("unroll (L <= 3 ? 2 * L + 1 : 1)")                                                  \
+            for (int ky = -L; ky <= L; ++ky)                                                            \
+                pdm3_pass<L, UNI, ST>(tile + (warp + L - ky) * ROW_SLOTS + (HG + lane) * GS,           \
+                                      (TB) + (ky + L) * (L + 1), toff, acc_a, acc_b);                   \
+        }
         if (staged) {
             if (uni) { PDM3_PASSES(true, true, slice) } else { PDM3_PASSES(false, true, slice) }
         } else {

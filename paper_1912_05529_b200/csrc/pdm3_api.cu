@@ -19,7 +19,7 @@ struct pdm3_plan {
     float *d_omega, *d_q, *d_partial;
     float4 *d_tab;
     float2 *d_plane[2];
-    int qstride, wgroups, smem_bytes, ctas_per_sm, grid, slice_rows;
+    int qstride, wgroups, smem_bytes, ctas_per_sm, grid, slice_rows, sym2;
     double workspace_bytes;
 };
 
@@ -41,10 +41,11 @@ static int pdm3_kernel_half_length(int L)
 #undef X
     return 0;
 }
-static pdm3_fn pdm3_kernel_for(int Lk, bool wide)
+static pdm3_fn pdm3_kernel_for(int Lk, bool wide, bool sym2)
 {
     switch (Lk) {
-#define X(LL) case LL: return wide ? pdm3_step<LL, 2> : pdm3_step<LL, 1>;
+#define X(LL) case LL: return sym2 ? (wide ? pdm3_step<LL, 2, true> : pdm3_step<LL, 1, true>) \
+                                   : (wide ? pdm3_step<LL, 2, false> : pdm3_step<LL, 1, false>);
         PDM3_FOR_EACH_L(X)
 #undef X
     default: return nullptr;
@@ -81,7 +82,7 @@ extern "C" int pdm3_create(pdm3_plan **out, int nx, int ny, int nz, int nw, floa
     if (nx <= 0 || ny <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0)
         return PDM_ERR_INVALID_ARG;
     if (!(tab_du > 0.0) || !std::isfinite(tab_du) || !(dz > 0.f) || !std::isfinite(dz)) return PDM_ERR_INVALID_ARG;
-    if (flags & ~PDM_FORCE_GENERAL) return PDM_ERR_INVALID_ARG;
+    if (flags & ~(PDM_FORCE_GENERAL | PDM_REQUIRE_SYMMETRIC)) return PDM_ERR_INVALID_ARG;
     const int L = (ntaps - 1) / 2, Lk = pdm3_kernel_half_length(L);
     if (!Lk) return PDM_ERR_UNSUPPORTED;                    // longer than the longest unrolled 2-D kernel (15 x 15)
     const double slab = (double)ny * (double)nx;
@@ -125,16 +126,39 @@ extern "C" int pdm3_create(pdm3_plan **out, int nx, int ny, int nz, int nw, floa
         volatile float prod = wmax * qmax;
         if (!std::isfinite(qmax) || !(prod < 2.0e9f) || lrintf(prod) > ntab - 1) { pdm3_free(p); return PDM_ERR_TABLE_RANGE; }
     }
-    // table rows as (W[ky][kx], W[ky][-kx]) units, kx = 0..Lk, ky = -Lk..Lk (zero taps beyond L)
-    const int units = (2 * Lk + 1) * (Lk + 1);
-    std::vector<float4> tab((size_t)ntab * units, make_float4(0.f, 0.f, 0.f, 0.f));
-    for (int j = 0; j < ntab; ++j)
-        for (int ky = -L; ky <= L; ++ky)
-            for (int k = 0; k <= L; ++k) {
-                const pdm_c64 a = table[((size_t)j * ntaps + (L + ky)) * ntaps + (L + k)];
-                const pdm_c64 b = table[((size_t)j * ntaps + (L + ky)) * ntaps + (L - k)];
-                tab[(size_t)j * units + (size_t)(ky + Lk) * (Lk + 1) + k] = make_float4(a.re, a.im, b.re, b.im);
+    // W[ky][kx] == W[-ky][kx] == W[ky][-kx] bit for bit in every row: the folded kernels (L+1 passes over
+    // row sums, 1 FADD2 + 2 FFMA2 per tap pair); otherwise the general ones (Eq. (1) literally)
+    bool sym2 = true;
+    for (int j = 0; j < ntab && sym2; ++j)
+        for (int ky = -L; ky <= L && sym2; ++ky)
+            for (int kx = -L; kx <= L; ++kx) {
+                const pdm_c64 *a = &table[((size_t)j * ntaps + (L + ky)) * ntaps + (L + kx)];
+                const pdm_c64 *b = &table[((size_t)j * ntaps + (L - ky)) * ntaps + (L + kx)];
+                const pdm_c64 *c = &table[((size_t)j * ntaps + (L + ky)) * ntaps + (L - kx)];
+                if (memcmp(a, b, sizeof(pdm_c64)) != 0 || memcmp(a, c, sizeof(pdm_c64)) != 0) { sym2 = false; break; }
             }
+    if (flags & PDM_REQUIRE_SYMMETRIC) { if (!sym2) { pdm3_free(p); return PDM_ERR_TABLE_ASYMMETRIC; } }
+    p->sym2 = sym2 ? 1 : 0;
+    const int ku = sym2 ? (Lk + 2) / 2 : Lk + 1;
+    const int units = (sym2 ? Lk + 1 : 2 * Lk + 1) * ku;
+    std::vector<float4> tab((size_t)ntab * units, make_float4(0.f, 0.f, 0.f, 0.f));
+    for (int j = 0; j < ntab; ++j) {
+        if (sym2) {                                        // units (W[ky][2t], W[ky][2t+1]), ky = 0..L
+            for (int ky = 0; ky <= L; ++ky)
+                for (int k = 0; k <= L; ++k) {
+                    const pdm_c64 a = table[((size_t)j * ntaps + (L + ky)) * ntaps + (L + k)];
+                    float4 &d = tab[(size_t)j * units + (size_t)ky * ku + k / 2];
+                    if (k & 1) { d.z = a.re; d.w = a.im; } else { d.x = a.re; d.y = a.im; }
+                }
+        } else {                                           // units (W[ky][kx], W[ky][-kx]), kx = 0..L, ky = -L..L
+            for (int ky = -L; ky <= L; ++ky)
+                for (int k = 0; k <= L; ++k) {
+                    const pdm_c64 a = table[((size_t)j * ntaps + (L + ky)) * ntaps + (L + k)];
+                    const pdm_c64 b = table[((size_t)j * ntaps + (L + ky)) * ntaps + (L - k)];
+                    tab[(size_t)j * units + (size_t)(ky + Lk) * (Lk + 1) + k] = make_float4(a.re, a.im, b.re, b.im);
+                }
+        }
+    }
 
     int rc;
 #define PDM3_TRY(call) do { if ((rc = (call)) != PDM_OK) { pdm3_free(p); return rc; } } while (0)
@@ -146,14 +170,14 @@ extern "C" int pdm3_create(pdm3_plan **out, int nx, int ny, int nz, int nw, floa
     // models where (nearly) every sample has its own row: a per-tile, per-frequency slice of the table in
     // shared memory (32 KB, 64 KB for the long operators) instead of gathering rows through L1
     if (varied * 4 > (size_t)nz * ny * nx) {
-        const int units_p = ((2 * Lk + 1) * (Lk + 1)) | 1;
+        const int units_p = units | 1;
         const int slice_bytes = (Lk <= 3 ? 32 : 64) * 1024;
         p->slice_rows = slice_bytes / (units_p * (int)sizeof(float4));
         p->smem_bytes += p->slice_rows * units_p * (int)sizeof(float4);
     }
     int per_sm = 0;
     for (int wide = 0; wide < 2; ++wide) {
-        pdm3_fn fn = pdm3_kernel_for(Lk, wide != 0);
+        pdm3_fn fn = pdm3_kernel_for(Lk, wide != 0, sym2);
         cudaError_t e = cudaFuncSetAttribute((const void *)fn, cudaFuncAttributeMaxDynamicSharedMemorySize, p->smem_bytes);
         if (e == cudaSuccess)
             e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)fn, PDM3_THREADS, (size_t)p->smem_bytes);
@@ -191,7 +215,7 @@ extern "C" int pdm3_migrate(pdm3_plan *p, const pdm_c64 *P0_dev, float *image_de
     a.slice_rows = p->slice_rows;
     // 16-byte copies and stores need every plane row 16-byte aligned: nx even and an aligned P0
     const bool wide = (p->nx % 2 == 0) && (((uintptr_t)P0_dev & 15u) == 0);
-    pdm3_fn fn = pdm3_kernel_for(p->Lk, wide);
+    pdm3_fn fn = pdm3_kernel_for(p->Lk, wide, p->sym2 != 0);
     dim3 grid((p->nx + PDM3_TX - 1) / PDM3_TX, (p->ny + PDM3_TY - 1) / PDM3_TY, p->wgroups);
     const float2 *src = reinterpret_cast<const float2 *>(P0_dev);
     for (int z = 0; z < p->nz; ++z) {
@@ -216,10 +240,11 @@ extern "C" int pdm3_get_info(const pdm3_plan *p, pdm_info *out)
     out->grid_ctas = p->grid; out->threads_per_cta = PDM3_THREADS; out->ctas_per_sm = p->ctas_per_sm;
     out->smem_bytes = p->smem_bytes; out->launches_per_migrate = p->nz + 1;
     out->sm_count = p->sm_count; out->last_cuda_error = p->last_cuda_error;
-    out->table_symmetric = 0;
+    out->table_symmetric = p->sym2;
     out->samples = (double)p->nx * (double)p->ny * (double)p->nz * (double)p->nw;
     out->counted_flops = 8.0 * p->ntaps * p->ntaps * out->samples;
-    out->executed_lane_ops = 4.0 * (2 * p->Lk + 1) * (2 * p->Lk + 1) * out->samples;
+    out->executed_lane_ops = (p->sym2 ? (double)(p->Lk + 1) * (6.0 * p->Lk + 4.0)
+                                      : 4.0 * (2 * p->Lk + 1) * (2 * p->Lk + 1)) * out->samples;
     out->workspace_bytes = p->workspace_bytes;
     return PDM_OK;
 }

@@ -435,10 +435,10 @@ def random_problem(seed: int, nx: int, nz: int, nw: int, ntaps: int, ntab: int =
 
 
 def random_problem_3d(seed: int, nx: int, ny: int, nz: int, nw: int, ntaps: int, ntab: int = 64,
-                      model: str = "field"):
+                      model: str = "field", symmetric: bool = False):
     """Seeded 3-D problem: velocity [nz, ny, nx] ('const' | 'layers' | 'field' = smooth in
     x, varying with y and z | 'white'), a random GENERAL 2-D table [ntab, ntaps, ntaps] scaled so that
-    sum |W| < 1 (stable for any index pattern), Gaussian P0 [nw, ny, nx]."""
+    sum |W| < 1 (stable for any index pattern; `symmetric`: mirrored in kx and in ky), Gaussian P0 [nw, ny, nx]."""
     rng = np.random.default_rng([seed, nx, ny, nz, nw, ntaps])
     dz = 10.0
     if model == "const":
@@ -459,6 +459,11 @@ def random_problem_3d(seed: int, nx: int, ny: int, nz: int, nw: int, ntaps: int,
     du = _table_du(omega, dz, v_in, ntab)
     table = (rng.standard_normal((ntab, ntaps, ntaps)) + 1j * rng.standard_normal((ntab, ntaps, ntaps)))
     table = (table / (np.abs(table).sum(axis=(1, 2), keepdims=True) * 1.02)).astype(np.complex64)
+    if symmetric:                                   # W[ky][kx] = W[-ky][kx] = W[ky][-kx], bit for bit
+        L = (ntaps - 1) // 2
+        q = table[:, L:, L:]
+        table = np.ascontiguousarray(np.concatenate([np.concatenate([q[:, :0:-1, :0:-1], q[:, :0:-1, :]], 2),
+                                                     np.concatenate([q[:, :, :0:-1], q], 2)], 1))
     P0 = np.empty((nw, ny, nx), dtype=np.complex64)
     P0.real = rng.standard_normal((nw, ny, nx), dtype=np.float32)
     P0.imag = rng.standard_normal((nw, ny, nx), dtype=np.float32)

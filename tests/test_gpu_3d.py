@@ -46,6 +46,32 @@ def test_3d_matches_oracle(pdm, model, nx, ny, nz, nw, ntaps):
     assert np.isfinite(a.cpu().numpy()).all() and rel <= 1e-4 and mx <= 1e-3, (rel, mx, info)
 
 
+@pytest.mark.parametrize("model,nx,ny,nz,nw,ntaps", [
+    ("field", 70, 19, 5, 3, 3), ("white", 300, 20, 4, 5, 7), ("layers", 513, 9, 6, 4, 5),
+    ("const", 64, 64, 3, 2, 15), ("field", 260, 33, 3, 9, 9), ("layers", 1, 5, 3, 2, 5),
+])
+def test_3d_doubly_symmetric_operators_run_folded(pdm, model, nx, ny, nz, nw, ntaps):
+    """W[ky][kx] = W[-ky][kx] = W[ky][-kx] bit for bit: the folded kernels (rows y-ky and y+ky added while
+    loaded, x-sum folded).  The oracle always applies the full (2L+1)^2 operator, so a folding mistake
+    (a row pair counted twice, the centre row added to itself, a wrong tap pairing) fails here."""
+    import torch
+    cfg = pdm_inputs.random_problem_3d(17, nx, ny, nz, nw, ntaps, model=model, symmetric=True)
+    t = cfg["table"]
+    assert np.array_equal(t, t[:, ::-1, :]) and np.array_equal(t, t[:, :, ::-1])
+    ref = oracle.migrate3d(cfg)
+    with pdm.Plan3D.from_config(cfg, pdm.PDM_REQUIRE_SYMMETRIC) as plan:
+        info = plan.info
+        assert info["table_symmetric"] == 1
+        img = plan.migrate(torch.from_numpy(cfg["P0"]).cuda())
+        torch.cuda.synchronize()
+    rel, mx = _errors(img.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx, info)
+    gen = pdm_inputs.random_problem_3d(17, nx, ny, nz, nw, ntaps, model=model)
+    rc, h = pdm.pdm3_create(gen["nx"], gen["ny"], gen["nz"], gen["nw"], gen["dz"], gen["omega"], gen["velocity"],
+                            gen["table"], gen["du"], pdm.PDM_REQUIRE_SYMMETRIC)
+    assert rc == (pdm.PDM_ERR_TABLE_ASYMMETRIC if ntaps > 1 else pdm.PDM_OK) and h is None
+
+
 def test_3d_force_general_and_unaligned_input(pdm):
     import torch
     cfg = pdm_inputs.random_problem_3d(9, 200, 12, 4, 3, 5, model="layers")
