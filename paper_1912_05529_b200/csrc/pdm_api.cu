@@ -1101,14 +1101,15 @@ struct pdm_tf {
     int *d_bins;
     float2 *d_tw;
     // nt a power of two: real FFT per trace (kern_fft.cuh); else the contraction (kern_tf.cuh)
-    int fft, log2nt, fft_S, fft_ntw, fft_smem;
+    int fft, log2nt, fft_S, fft_ntw, fft_smem, fft_grid;
     float2 *d_ftw;
+    int2 *d_binpos;
 };
 
 extern "C" int pdm_tf_destroy(pdm_tf *tf)
 {
     if (!tf) return PDM_OK;
-    cudaFree(tf->d_bins); cudaFree(tf->d_tw); cudaFree(tf->d_ftw);
+    cudaFree(tf->d_bins); cudaFree(tf->d_tw); cudaFree(tf->d_ftw); cudaFree(tf->d_binpos);
     delete tf;
     return PDM_OK;
 }
@@ -1168,12 +1169,27 @@ extern "C" int pdm_tf_create(pdm_tf **out, int nt, int nx, int nw, const int *bi
         while (S > 1 && (S * np + ftw.size()) * sizeof(float2) > (size_t)160 * 1024) S >>= 1;
         while (S > 1 && S / 2 >= (nx + 1) / 2) S >>= 1;    // no more pairs than the section has
         const size_t smem = (S * np + ftw.size()) * sizeof(float2);
+        // where the in-place DIF leaves bin k: radix-4 digits reversed, then the radix-2 bit; padded index
+        auto pos_of = [&](int k) {
+            int pos = 0, rem = lg;
+            while (rem >= 2) { rem -= 2; pos += (k & 3) << rem; k >>= 2; }
+            if (rem == 1) pos += k & 1;
+            return pos + (pos >> 4);
+        };
+        std::vector<int2> binpos(nw);
+        for (int j = 0; j < nw; ++j) binpos[j] = make_int2(pos_of(bins[j]), pos_of((nt - bins[j]) & (nt - 1)));
         if (smem <= (size_t)prop.sharedMemPerBlockOptin - 1024 &&
+            cudaMalloc((void **)&tf->d_binpos, (size_t)nw * sizeof(int2)) == cudaSuccess &&
+            cudaMemcpy(tf->d_binpos, binpos.data(), (size_t)nw * sizeof(int2), cudaMemcpyHostToDevice) == cudaSuccess &&
             cudaMalloc((void **)&tf->d_ftw, ftw.size() * sizeof(float2)) == cudaSuccess &&
             cudaMemcpy(tf->d_ftw, ftw.data(), ftw.size() * sizeof(float2), cudaMemcpyHostToDevice) == cudaSuccess &&
             cudaFuncSetAttribute((const void *)pdm_fft_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                  (int)smem) == cudaSuccess) {
             tf->fft = 1; tf->log2nt = lg; tf->fft_S = S; tf->fft_ntw = (int)ftw.size(); tf->fft_smem = (int)smem;
+            int per_sm = 1;                                // persistent CTAs: the twiddle tables are loaded once each
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, (const void *)pdm_fft_kernel, PDM_FFT_THREADS,
+                                                              smem) != cudaSuccess || per_sm < 1) { cudaGetLastError(); per_sm = 1; }
+            tf->fft_grid = prop.multiProcessorCount * per_sm;
         } else {
             cudaGetLastError();                            // fall through to the contraction form
         }
@@ -1206,13 +1222,14 @@ extern "C" int pdm_tf_forward(pdm_tf *tf, const float *section_dev, pdm_c64 *P0_
     if (tf->fft) {
         pdm_fft_params f;
         f.section = section_dev; f.out = reinterpret_cast<float2 *>(P0_dev);
-        f.bins = tf->d_bins; f.tw = tf->d_ftw;
+        f.binpos = tf->d_binpos; f.tw = tf->d_ftw;
         f.nt = tf->nt; f.log2nt = tf->log2nt; f.nx = tf->nx; f.nw = tf->nw;
         f.S = tf->fft_S; f.ntw = tf->fft_ntw;
         f.pair_loads = (tf->nx % 2 == 0 && ((uintptr_t)section_dev & 7u) == 0) ? 1 : 0;
         f.wide_out = (tf->nx % 2 == 0 && ((uintptr_t)P0_dev & 15u) == 0) ? 1 : 0;
         const int per_cta = 2 * tf->fft_S;
-        pdm_fft_kernel<<<(tf->nx + per_cta - 1) / per_cta, PDM_FFT_THREADS, tf->fft_smem, (cudaStream_t)cuda_stream>>>(f);
+        const int ntiles = (tf->nx + per_cta - 1) / per_cta;
+        pdm_fft_kernel<<<std::min(ntiles, tf->fft_grid), PDM_FFT_THREADS, tf->fft_smem, (cudaStream_t)cuda_stream>>>(f);
         if (cudaGetLastError() != cudaSuccess) return PDM_ERR_CUDA;
         return PDM_OK;
     }
