@@ -115,3 +115,31 @@ def test_3d_at_bench_tile_counts(pdm, model, ntaps):
         torch.cuda.synchronize()
     rel, mx = _errors(img.cpu().numpy(), ref)
     assert rel <= 1e-4 and mx <= 1e-3, (rel, mx)
+
+
+def test_3d_and_prestack_are_cuda_graph_capturable(pdm):
+    """pdm3_migrate and pdm_migrate_shot only enqueue work (per-step launches; the cooperative packed
+    kernel plus its interleave kernel): capture and replay."""
+    import torch
+    cfg3 = pdm_inputs.random_problem_3d(21, 130, 17, 4, 3, 5, model="field")
+    cfg2 = pdm_inputs.random_problem(22, 900, 7, 6, 15, model="field")
+    rng = np.random.default_rng(1)
+    S0 = (rng.standard_normal((6, 900)) + 1j * rng.standard_normal((6, 900))).astype(np.complex64)
+    with pdm.Plan3D.from_config(cfg3) as p3, pdm.Plan.from_config(cfg2, pdm.PDM_PRESTACK) as p2:
+        a3 = torch.from_numpy(cfg3["P0"]).cuda()
+        s, r = torch.from_numpy(S0).cuda(), torch.from_numpy(cfg2["P0"]).cuda()
+        ref3 = p3.migrate(a3).clone()
+        ref2 = p2.migrate_shot(s, r).clone()
+        img3, img2 = torch.zeros_like(ref3), torch.zeros_like(ref2)
+        torch.cuda.synchronize()
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=st):
+                p3.migrate(a3, img3, stream=st)
+                p2.migrate_shot(s, r, img2, stream=st)
+        img3.zero_(); img2.zero_()
+        torch.cuda.synchronize()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(img3, ref3) and torch.equal(img2, ref2)
