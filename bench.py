@@ -214,6 +214,23 @@ def time_migrate(plan, P0, image, stream, flush, torch, steps: int, warmup: int 
     return ms
 
 
+def oracle_one_thread(k: int, max_lines: int = 12):
+    """the oracle on ONE host thread for the small configs (a fresh process with
+    OMP_NUM_THREADS=1; a bounded sample of evenly spaced lines) -> samples/s, or None."""
+    code = (f"import sys, time, json, numpy as np; sys.path.insert(0, {ROOT!r}); import oracle, pdm_inputs;"
+            f"c = pdm_inputs.make_config({k}); n = min(c['nw'], {max_lines});"
+            "idx = np.unique(np.linspace(0, c['nw'] - 1, n).round().astype(np.int32));"
+            "oracle.migrate(c, omega_index=idx[:1]); t = time.perf_counter(); oracle.migrate(c, omega_index=idx);"
+            "dt = time.perf_counter() - t;"
+            "print(json.dumps({'v': float(idx.size) * c['nx'] * c['nz'] / dt, 'lines': int(idx.size), 'threads': oracle.num_threads()}))")
+    try:
+        out = subprocess.run([sys.executable, "-c", code], env=dict(os.environ, OMP_NUM_THREADS="1"),
+                             capture_output=True, text=True, timeout=300)
+        return json.loads(out.stdout.strip().splitlines()[-1])
+    except Exception:                                       # a reported baseline only: never fail the bench over it
+        return None
+
+
 def other_configs(pdm, torch, dev, stream, flush):
     """The regimes the headline workload does not show, measured in the same run (a few seconds):
     configs[0..2] and two configs[4] points where every sample has its own table row (tap-gather
@@ -239,6 +256,11 @@ def other_configs(pdm, torch, dev, stream, flush):
                      "frac_fp32_peak_counted": sps * 8 * cfg["ntaps"] / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
                      "frac_hbm_16B_per_sample_of_measured":
                          (sps * 16 / (measured_hbm_gbs()[0] * 1e9)) if info["path"] == pdm.PDM_PATH_TILED else None})
+        if name in ("configs[0]", "configs[1]"):
+            o = oracle_one_thread(int(name[8]))
+            if o:
+                rows[-1]["oracle_one_thread"] = {"value": o["v"], "unit": UNIT, "cores": o["threads"],
+                                                 "sample": f"{o['lines']} evenly spaced omega lines"}
         del P0, image
     return rows
 
