@@ -604,7 +604,11 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
         const bool dense = nw >= 2 * PDM_PACK_W && sigma <= 1.3f;
         const long long items = (long long)((nw + PDM_PACK_W - 1) / PDM_PACK_W) * ((nx + 447) / 448);
         // (sparse lists -- more than ~6 rows between adjacent lines -- keep the x-tiled form: 0.8-0.95x there)
-        if ((p->path == PDM_PATH_TILED && sigma <= 6.f) || (dense && nx >= 3072 && items >= 3LL * p->sm_count)) {
+        // dense lists, measured against the SMEM form (field model, nw = 1024 / 2048): 15 taps win from nx = 4096
+        // (0.88x at 3072), longer filters from nx = 3072 (1.0-1.25x) and, with enough items per SM, from 2048
+        const int min_nx = Lk <= 7 ? 4096 : 2048;
+        const long long min_items = (long long)p->sm_count * (nx >= 3072 ? 3 : (Lk >= 25 ? 4 : 8));
+        if ((p->path == PDM_PATH_TILED && sigma <= 6.f) || (dense && nx >= min_nx && items >= min_items)) {
             rc = build_packed(p, omega, q, half, Lk, HG);
             if (rc == PDM_OK) packed_done = true;
             else if (rc != PDM_ERR_UNSUPPORTED) return rc;
