@@ -41,6 +41,13 @@ def _load():
             ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_double,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int,
             ctypes.c_void_p, ctypes.c_void_p]
+        lib.pdm_oracle_migrate_taper.restype = ctypes.c_int
+        lib.pdm_oracle_migrate_taper.argtypes = [
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p,
+            ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_double,
+            ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
+            ctypes.c_void_p, ctypes.c_void_p]
         lib.pdm_oracle_index.restype = ctypes.c_int
         lib.pdm_oracle_index.argtypes = [ctypes.c_float, ctypes.c_float, ctypes.c_double,
                                          ctypes.c_double, ctypes.c_int]
@@ -71,7 +78,7 @@ def table_index(omega, velocity, dz: float, du: float, ntab: int) -> int:
                                         float(dz), float(du), int(ntab)))
 
 
-def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field):
+def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field, ntaper=0):
     lib = _load()
     omega = np.ascontiguousarray(omega, dtype=np.float32)
     velocity = np.ascontiguousarray(velocity, dtype=np.float32)
@@ -87,27 +94,35 @@ def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field
         assert nsub > 0 and sub.min() >= 0 and sub.max() < nw
     image = np.zeros((nz, nx), dtype=np.float64)
     field = np.zeros((nlines, nx), dtype=np.complex128) if want_field else None
-    rc = lib.pdm_oracle_migrate(
-        nx, nz, nw, float(dz), omega.ctypes.data, velocity.ctypes.data,
-        table.ctypes.data, ntab, ntaps, float(du), P0.ctypes.data,
-        None if sub is None else sub.ctypes.data, nsub,
-        image.ctypes.data, None if field is None else field.ctypes.data)
+    if ntaper:
+        rc = lib.pdm_oracle_migrate_taper(
+            nx, nz, nw, float(dz), omega.ctypes.data, velocity.ctypes.data,
+            table.ctypes.data, ntab, ntaps, float(du), P0.ctypes.data,
+            None if sub is None else sub.ctypes.data, nsub, int(ntaper),
+            image.ctypes.data, None if field is None else field.ctypes.data)
+    else:
+        rc = lib.pdm_oracle_migrate(
+            nx, nz, nw, float(dz), omega.ctypes.data, velocity.ctypes.data,
+            table.ctypes.data, ntab, ntaps, float(du), P0.ctypes.data,
+            None if sub is None else sub.ctypes.data, nsub,
+            image.ctypes.data, None if field is None else field.ctypes.data)
     if rc != 0:
         raise RuntimeError(f"pdm_oracle_migrate failed with code {rc}")
     return image, field
 
 
-def migrate(cfg: dict, omega_index=None) -> np.ndarray:
-    """image float64 [nz, nx] for a workload dict (pdm_inputs layout); optional omega subset."""
+def migrate(cfg: dict, omega_index=None, ntaper: int = 0) -> np.ndarray:
+    """image float64 [nz, nx] for a workload dict (pdm_inputs layout); optional omega subset;
+    ntaper > 0: the absorbing edge-taper variant of R5 (reading R5b)."""
     img, _ = _run(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dz"], cfg["omega"], cfg["velocity"],
-                  cfg["table"], cfg["du"], cfg["P0"], omega_index, False)
+                  cfg["table"], cfg["du"], cfg["P0"], omega_index, False, ntaper)
     return img
 
 
-def migrate_field(cfg: dict, omega_index=None):
+def migrate_field(cfg: dict, omega_index=None, ntaper: int = 0):
     """(image, final wavefield complex128 [nlines, nx]) -- the field after the last depth step."""
     return _run(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dz"], cfg["omega"], cfg["velocity"],
-                cfg["table"], cfg["du"], cfg["P0"], omega_index, True)
+                cfg["table"], cfg["du"], cfg["P0"], omega_index, True, ntaper)
 
 
 def migrate_shot(cfg: dict, S0, R0, image=None) -> np.ndarray:

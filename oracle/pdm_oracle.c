@@ -40,7 +40,8 @@
  * P5 point-diffractor focusing, P7 superposition, P8 w-additivity/permutation, P9 mirror,
  * P10 energy non-growth, P11 shift invariance, P12a index rule (the function), P12b index rule
  * THROUGH the migrate loop (centre-tap-encodes-row table; a double product or a float-formed q
- * inside the loop fails it).  The file is also built with -fsanitize=address,undefined and run
+ * inside the loop fails it).  The edge-taper variant R5b (pdm_oracle_migrate_taper; the plain entry point
+ * is that function with ntaper = 0) has its own pins in tests/test_oracle_taper_pins.py.  The file is also built with -fsanitize=address,undefined and run
  * on ragged cases (tests/test_oracle_sanitize.py).  Parity unpinned by anything external: the
  * choices R5/R6/R7 (boundary, row<->depth, velocity row) and the absolute amplitude scale R10
  * -- fixed by DESIGN.md only (P5 accepts +-1 row, so it does not pin R6 to the row either).
@@ -98,6 +99,25 @@ int pdm_oracle_index(float omega, float velocity, double dz, double du, int ntab
  * complex double [nw][nx] (used by pins P3/P4/P10 which look at the field, not the image).
  * omega_subset: if nsub > 0, only lines omega_index[0..nsub) are migrated (bench sampling, P8).
  */
+/* R5 variant (reading R5b; the paper is silent on the lateral boundary): an absorbing
+ * cosine edge taper.  After every depth step the new field is multiplied by
+ *     t(x) = sin^2( (pi/2) (d+1)/(ntaper+1) ),  d = min(x, nx-1-x),  for d < ntaper;  t(x) = 1 otherwise
+ * BEFORE it is imaged and before the next step reads it.  ntaper = 0 is plain R5. */
+static double oracle_taper(int x, int nx, int ntaper)
+{
+    const int d = x < nx - 1 - x ? x : nx - 1 - x;
+    if (d >= ntaper) return 1.0;
+    const double s = sin(1.57079632679489661923 * (double)(d + 1) / (double)(ntaper + 1));
+    return s * s;
+}
+
+int pdm_oracle_migrate_taper(int nx, int nz, int nw, double dz,
+                             const float *omega, const float *velocity,
+                             const oracle_c64 *table, int ntab, int ntaps, double du,
+                             const oracle_c64 *P0,
+                             const int *omega_index, int nsub, int ntaper,
+                             double *image_out, double *wavefield_out);
+
 int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
                        const float *omega, const float *velocity,
                        const oracle_c64 *table, int ntab, int ntaps, double du,
@@ -105,7 +125,18 @@ int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
                        const int *omega_index, int nsub,
                        double *image_out, double *wavefield_out)
 {
-    if (nx <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0 ||
+    return pdm_oracle_migrate_taper(nx, nz, nw, dz, omega, velocity, table, ntab, ntaps, du, P0,
+                                    omega_index, nsub, 0, image_out, wavefield_out);
+}
+
+int pdm_oracle_migrate_taper(int nx, int nz, int nw, double dz,
+                             const float *omega, const float *velocity,
+                             const oracle_c64 *table, int ntab, int ntaps, double du,
+                             const oracle_c64 *P0,
+                             const int *omega_index, int nsub, int ntaper,
+                             double *image_out, double *wavefield_out)
+{
+    if (nx <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0 || ntaper < 0 ||
         !(du > 0.0) || !omega || !velocity || !table || !P0 || !image_out)
         return ORACLE_ERR_ARG;
     const int L = (ntaps - 1) / 2;
@@ -159,6 +190,10 @@ int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
                             double pr = P[2 * xs], pi = P[2 * xs + 1];
                             ar += wr * pr - wi * pi;
                             ai += wr * pi + wi * pr;
+                        }
+                        if (ntaper > 0) {                               /* R5b: absorbing edge taper */
+                            const double t = oracle_taper(x, nx, ntaper);
+                            ar *= t; ai *= t;
                         }
                         Pn[2 * x] = ar;                                 /* O8 */
                         Pn[2 * x + 1] = ai;
