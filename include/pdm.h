@@ -88,7 +88,13 @@ typedef enum {
 #define PDM_PRESTACK      (1u << 21) /* plan for pdm_migrate_shot (shot-profile prestack migration,    */
                                     /* PAPER.md:151): always the PDM_PATH_PACKED form (AUTO or PACKED   */
                                     /* path bits), any table; pdm_migrate refuses such a plan           */
-#define PDM_FLAGS_VALID  0x003FFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
+#define PDM_TAPER_SHIFT   22         /* bits 22-29: absorbing edge taper over n = 1..255 samples per side  */
+                                    /* (variant R5b of the zero edges R5; the paper is silent on the     */
+                                    /* boundary): after every step the new field is multiplied by        */
+                                    /* t(x) = sin^2((pi/2)(d+1)/(n+1)), d = min(x, nx-1-x) < n.  Always   */
+                                    /* the PDM_PATH_PACKED form (AUTO or PACKED path bits); not with      */
+                                    /* PDM_PRESTACK.  0 = plain R5                                        */
+#define PDM_FLAGS_VALID  0x3FFFFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
 
 typedef struct {
     int    path;                 /* PDM_PATH_* actually chosen                                      */

@@ -25,7 +25,7 @@ PDM_ERR_CUDA = -6
 PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER, PDM_PATH_PACKED = 0, 1, 2, 3, 4, 5
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC, PDM_PRESTACK = 1 << 6, 1 << 7, 1 << 20, 1 << 21
-PDM_THREADS_SHIFT, PDM_CTAS_SHIFT = 8, 16
+PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TAPER_SHIFT = 8, 16, 22
 
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_migrate_shot", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",

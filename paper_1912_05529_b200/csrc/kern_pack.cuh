@@ -60,6 +60,8 @@ struct alignas(64) pdm_pack_params {
     int xcorr;                    // prestack: lines 2i / 2i+1 are the receiver field and the conjugated source field of
                                   // frequency i; the image is sum Re(U R) over the pairs instead of sum Re P (R17)
     int accumulate;               // add to the image instead of overwriting it (several shots)
+    int ntaper;                   // R5b: absorbing edge taper over this many samples per side (0: plain R5)
+    const float *taper;           // [ntaper] t(d) = sin^2((pi/2)(d+1)/(ntaper+1)), d = distance to the nearer edge
 };
 
 __device__ __forceinline__ unsigned pdm_smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
@@ -275,6 +277,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_cons
 #pragma unroll
                         for (int r = 0; r < R; ++r)
                             if ((unsigned)(xg + r) >= (unsigned)p.nx) out[r] = make_float2(0.f, 0.f);
+                    }
+                    if (p.ntaper > 0 && (xg < p.ntaper || xg + R > p.nx - p.ntaper)) {   // R5b (edge groups only)
+#pragma unroll
+                        for (int r = 0; r < R; ++r) {
+                            const int x = xg + r, d = min(x, p.nx - 1 - x);
+                            if (d >= 0 && d < p.ntaper) {
+                                const float t = __ldg(p.taper + d);
+                                out[r].x *= t; out[r].y *= t;
+                            }
+                        }
                     }
                     const bool central = g >= gc0 && g < gc1;
                     if (!last_step) {

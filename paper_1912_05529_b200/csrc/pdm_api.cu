@@ -60,7 +60,7 @@ static void free_plan(pdm_plan *p)
     cudaFree(p->d_plane[0]); cudaFree(p->d_plane[1]); cudaFree(p->d_flags);
     cudaFree(p->d_handoff); cudaFree(p->d_segs); cudaFree(p->d_segoff);
     cudaFree(p->d_stage_p0); cudaFree(p->d_stage_img);
-    cudaFree(p->d_packw); cudaFree(p->d_tileq); cudaFree(p->d_tile_ctas);
+    cudaFree(p->d_packw); cudaFree(p->d_tileq); cudaFree(p->d_tile_ctas); cudaFree(p->d_taper);
     for (int i = 0; i < 3; ++i) if (p->ev[i]) cudaEventDestroy(p->ev[i]);
     delete p;
 }
@@ -130,6 +130,8 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
     // prestack plans carry two lines per frequency (receiver field, conjugated source field): R17
     const bool prestack = (flags & PDM_PRESTACK) != 0;
     if (prestack && path != PDM_PATH_AUTO && path != PDM_PATH_PACKED) return PDM_ERR_INVALID_ARG;
+    const int ntaper = (int)((flags >> PDM_TAPER_SHIFT) & 0xFFu);       // R5b: packed form only
+    if (ntaper && (prestack || (path != PDM_PATH_AUTO && path != PDM_PATH_PACKED))) return PDM_ERR_INVALID_ARG;
     std::vector<float> omega2;
     if (prestack) {
         if ((double)2 * nw * (double)nx > 2.0e9) return PDM_ERR_UNSUPPORTED;
@@ -142,6 +144,7 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
     if (!p) return PDM_ERR_NOMEM;
     memset(p, 0, sizeof(*p));
     p->prestack = prestack ? 1 : 0;
+    p->ntaper = ntaper;
     p->nx = nx; p->nz = nz; p->nw = nw; p->ntab = ntab; p->ntaps = ntaps; p->L = L;
     p->dx = dx; p->dz = dz; p->du = tab_du; p->flags = flags;
     p->sym = symmetric ? 1 : 0;
@@ -416,6 +419,14 @@ static int build_packed(pdm_plan *p, const float *omega, const std::vector<float
         PDM_CUDA(p, cudaMemset(p->d_plane[i], 0, (size_t)nw * p->nxp * sizeof(float2)));
         if ((rc = make_plane_map(p, &p->tmap_plane[i], p->d_plane[i], p->nxp, nw, BW)) != PDM_OK) return rc;
     }
+    if (p->ntaper) {                                       // R5b weights, formed in double
+        std::vector<float> tp(p->ntaper);
+        for (int d = 0; d < p->ntaper; ++d) {
+            const double sn = sin(1.57079632679489661923 * (double)(d + 1) / (double)(p->ntaper + 1));
+            tp[d] = (float)(sn * sn);
+        }
+        if ((rc = dev_upload(p, &p->d_taper, tp.data(), tp.size())) != PDM_OK) return rc;
+    }
     p->path = PDM_PATH_PACKED;
     return PDM_OK;
 }
@@ -569,7 +580,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     if (want == PDM_PATH_SMEM && !lines_fit) return PDM_ERR_UNSUPPORTED;
     if (want == PDM_PATH_TILED && !have_L) return PDM_ERR_UNSUPPORTED;  // (tiled_kernel_for has the same L list)
     if (want == PDM_PATH_PACKED && !have_L) return PDM_ERR_UNSUPPORTED;
-    if (p->prestack) {
+    if (p->prestack || p->ntaper) {
         if (!have_L) return PDM_ERR_UNSUPPORTED;
         p->path = PDM_PATH_PACKED;
     } else if (want == PDM_PATH_AUTO)
@@ -597,7 +608,7 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     // most ~1 row apart) and replaces the x-tiled form in any case (measured on configs[4], field model:
     // 1.06-1.3x over the SMEM form at nx = 4096, 1.2-1.65x over the cluster-pair / x-tiled forms beyond)
     bool packed_done = false;
-    if (want == PDM_PATH_AUTO && !p->prestack && have_L && p->sym && p->contiguous_rows) {
+    if (want == PDM_PATH_AUTO && !p->prestack && !p->ntaper && have_L && p->sym && p->contiguous_rows) {
         float sigma = 0.f;                                  // table rows between adjacent lines of a pack
         for (int k = 0; k + 1 < nw; ++k)
             if ((k + 1) % PDM_PACK_W) sigma = std::max(sigma, fabsf(omega[k + 1] - omega[k]) * qmax);
@@ -908,6 +919,7 @@ static int migrate_impl(pdm_plan *p, const pdm_c64 *P0_dev, const pdm_c64 *src_d
         // the first depth block reads the caller's P0 through its own TMA descriptor when its rows are
         // 16-byte aligned (nx even and an aligned base); otherwise P0 is first repacked into a plane
         a.xcorr = p->prestack; a.accumulate = accumulate;
+        a.ntaper = p->ntaper; a.taper = p->d_taper;
         if (p->prestack) {                               // (receiver, conj source) line pairs into plane 1
             dim3 cg((p->nxp + 255) / 256, nw / 2);
             pdm_pack_interleave<<<cg, 256, 0, st>>>(P0, reinterpret_cast<const float2 *>(src_dev), p->d_plane[1],

@@ -15,6 +15,8 @@ struct pdm_plan {
     double du;
     unsigned flags;
     int path, taps_mode;
+    int ntaper;           // R5b edge taper width (packed form only)
+    float *d_taper;       // [ntaper]
     int prestack;         // PDM_PRESTACK: nw counts LINES = 2 x the caller's frequencies ((receiver, conj source) pairs)
     int sym;              // 1: table bitwise symmetric in k (folded kernels); 0: general kernels (8L+4 lane-ops)
     int device, sm_count, smem_optin;

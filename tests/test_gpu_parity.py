@@ -203,6 +203,31 @@ def test_packed_path_matches_oracle_for_every_block_depth(pdm, T, model, nx, nz,
     assert np.isfinite(a.cpu().numpy()).all() and rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info)
 
 
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps,n,T", [
+    ("field", 300, 21, 7, 15, 20, 0),       # one tile: both edges inside it
+    ("white", 1000, 13, 19, 25, 40, 2),     # three tiles: the taper zones sit in the first and the last
+    ("layers", 2501, 10, 9, 7, 255, 4),     # the widest taper; odd nx
+    ("const", 129, 17, 3, 51, 100, 1),      # taper zones overlap in the middle (n > nx/2)
+    ("field", 1900, 9, 16, 35, 1, 0),       # one sample per side
+])
+def test_edge_taper_variant_matches_oracle(pdm, model, nx, nz, nw, ntaps, n, T):
+    """Reading R5b (optional): absorbing cosine taper over n samples per side applied
+    after every depth step, in the packed form, against pdm_oracle_migrate_taper."""
+    cfg = pdm_inputs.random_problem(47, nx, nz, nw, ntaps, model=model)
+    flags = (n << pdm.PDM_TAPER_SHIFT) | ((pdm.PDM_PATH_PACKED | (T << pdm.PDM_CTAS_SHIFT)) if T else 0)
+    img, info = gpu_migrate(pdm, cfg, flags, want_info=True)
+    assert info["path"] == pdm.PDM_PATH_PACKED
+    ref = oracle.migrate(cfg, ntaper=n)
+    rel, mx = errors(img, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info)
+    plain = oracle.migrate(cfg)
+    assert np.abs(plain - ref).max() > 1e-3 * np.abs(ref).max()       # the taper does something here
+    args = (cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"], cfg["velocity"], cfg["table"], cfg["du"])
+    for bad in (pdm.PDM_PATH_SMEM, pdm.PDM_PATH_TILED, pdm.PDM_PRESTACK):
+        rc, h = pdm.pdm_create(*args, (n << pdm.PDM_TAPER_SHIFT) | bad)
+        assert rc == pdm.PDM_ERR_INVALID_ARG and h is None
+
+
 def test_packed_path_with_unaligned_p0_pointer(pdm):
     """Even nx but a P0 that is only 8-byte aligned: TMA cannot address it, so the library repacks it
     into its own plane first; same image bit for bit as the direct descriptor on an aligned P0."""
