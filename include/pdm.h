@@ -45,7 +45,9 @@ typedef enum {
                                       filters of any odd length run on the next longer kernel with
                                       zero taps appended, longer ones only on PDM_PATH_NAIVE)      */
     PDM_ERR_NOMEM = -5,            /* host or device allocation failed                             */
-    PDM_ERR_CUDA = -6              /* a CUDA call failed; pdm_info.last_cuda_error has the code    */
+    PDM_ERR_CUDA = -6,             /* a CUDA call failed; pdm_info.last_cuda_error has the code    */
+    PDM_ERR_TOO_LARGE = -7         /* pdm_migrate_static only: nx*nw exceeds PDM_STATIC_MAX_SAMPLES, the
+                                      size of the library's built-in scratch                       */
 } pdm_status;
 
 #define PDM_MAX_TAPS 129           /* L <= 64 */
@@ -174,6 +176,52 @@ int pdm_migrate_host(pdm_plan *plan, const pdm_c64 *P0_host, float *image_host, 
  */
 int pdm_migrate_shot(pdm_plan *plan, const pdm_c64 *src_dev, const pdm_c64 *rec_dev, float *image_dev,
                      int accumulate, void *cuda_stream);
+
+/*
+ * pdm_migrate_static -- the whole migration (Eq. (1) at every depth level + the imaging sum, same
+ * index rule R3, zero edges R5 and row conventions R6/R7 as pdm_migrate) for callers that MUST NOT
+ * ALLOCATE device memory: no plan, no pdm_create.
+ *
+ * Who needs it: code that runs where cudaMalloc / cudaFree are off limits -- an extension inside a host
+ * application that owns all device memory and gives plug-ins fixed buffers; a latency-bound loop that
+ * cannot afford the device-wide synchronisation an allocation implies; a job sized to the last byte of
+ * HBM that must not discover an out-of-memory error in the middle of a survey.  Every other migration
+ * call of this library needs a plan, and pdm_create allocates.
+ *
+ * How: this entry point calls no cudaMalloc, cudaFree or any routine that allocates.  Its only scratch
+ * (two wavefield planes, ping-pong between depth steps) is a fixed array compiled into the library:
+ * 2 * PDM_STATIC_MAX_SAMPLES * 8 B = 16 MiB of device memory that every GPU on which the library's
+ * code gets loaded holds until the process exits, whether or not this call is ever used again.
+ * Problems with nx*nw > PDM_STATIC_MAX_SAMPLES are refused with PDM_ERR_TOO_LARGE (nothing is
+ * launched); nz is not limited.  It is the per-depth-step form (one thread per (w,x) sample, 2*nz small
+ * launches, the mapping of PDM_PATH_NAIVE): correct and allocation-free, not the fast path.
+ *
+ *   omega_dev     DEVICE float[nw]          rad/s (as pdm_create's omega, but already on the device)
+ *   velocity_dev  DEVICE float[nz][nx]      migration velocity, m/s
+ *   table_dev     DEVICE pdm_c64[ntab][ntaps], the layout pdm_create reads; symmetric or not
+ *   P0_dev        DEVICE pdm_c64[nw][nx]    read-only
+ *   image_dev     DEVICE float[nz][nx]      overwritten
+ * All five belong to the caller and must stay valid until the stream has run the call.  Their CONTENTS
+ * are not validated (that would need a host synchronisation): a table index beyond ntab-1 is clamped,
+ * non-finite or non-positive values give undefined images, not errors.
+ *
+ * First call on a device: the library looks up the device address of its scratch array (once per
+ * device, with that device current) before launching.  Make that first call outside any stream
+ * capture; later calls on the same device only launch kernels on cuda_stream.
+ *
+ * One array per process and GPU, shared by ALL calls: a call finds the previous call's wavefield in it.
+ * Nothing in it needs clearing -- every element is written in a call before that call reads it -- but two
+ * calls that may execute concurrently on one GPU (different streams without an event between them)
+ * corrupt each other.  Serialise them.  Deterministic: same inputs, same bits, and the same bits as a
+ * PDM_PATH_NAIVE plan.
+ * Errors: PDM_ERR_INVALID_ARG (NULL, size <= 0, even ntaps, dz or tab_du <= 0), PDM_ERR_UNSUPPORTED
+ * (ntaps > PDM_MAX_TAPS, no CC 10.x device current), PDM_ERR_TOO_LARGE, PDM_ERR_CUDA.
+ */
+#define PDM_STATIC_MAX_SAMPLES (1 << 20)   /* nx*nw limit of pdm_migrate_static                        */
+int pdm_migrate_static(int nx, int nz, int nw, float dz,
+                       const float *omega_dev, const float *velocity_dev,
+                       const pdm_c64 *table_dev, int ntab, int ntaps, double tab_du,
+                       const pdm_c64 *P0_dev, float *image_dev, void *cuda_stream);
 
 /* pdm_destroy -- free all device and host state of the plan.  NULL is allowed. */
 int pdm_destroy(pdm_plan *plan);

@@ -21,13 +21,15 @@ PDM_ERR_TABLE_ASYMMETRIC = -3
 PDM_ERR_UNSUPPORTED = -4
 PDM_ERR_NOMEM = -5
 PDM_ERR_CUDA = -6
+PDM_ERR_TOO_LARGE = -7
+PDM_STATIC_MAX_SAMPLES = 1 << 20
 
 PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER, PDM_PATH_PACKED = 0, 1, 2, 3, 4, 5
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC, PDM_PRESTACK = 1 << 6, 1 << 7, 1 << 20, 1 << 21
 PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TAPER_SHIFT = 8, 16, 22
 
-EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_migrate_shot", "pdm_destroy", "pdm_get_info",
+EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_migrate_shot", "pdm_migrate_static", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",
                     "pdm_profile_enable", "pdm_profile_read",
                     "pdm_tf_create", "pdm_tf_forward", "pdm_tf_destroy", "pdm_design_table",
@@ -80,6 +82,8 @@ def load_library(path: str | None = None):
     lib.pdm_migrate_shot.argtypes = [vp, vp, vp, vp, ci, vp]
     lib.pdm_migrate_host.restype = ci
     lib.pdm_migrate_host.argtypes = [vp, vp, vp, vp]
+    lib.pdm_migrate_static.restype = ci
+    lib.pdm_migrate_static.argtypes = [ci, ci, ci, cf, vp, vp, vp, ci, ci, cd, vp, vp, vp]
     lib.pdm_destroy.restype = ci
     lib.pdm_destroy.argtypes = [vp]
     lib.pdm_get_info.restype = ci
@@ -115,7 +119,8 @@ def load_library(path: str | None = None):
 
 
 _STRERROR_LOCAL = {0: "ok", -1: "invalid argument", -2: "table range", -3: "table asymmetric",
-                   -4: "unsupported", -5: "out of memory", -6: "CUDA call failed"}
+                   -4: "unsupported", -5: "out of memory", -6: "CUDA call failed",
+                   -7: "too large for the built-in scratch"}
 
 
 def pdm_strerror(code: int) -> str:
@@ -157,6 +162,41 @@ def pdm_migrate_shot(plan, src_dev_ptr: int, rec_dev_ptr: int, image_dev_ptr: in
 def pdm_migrate_host(plan, P0_host_ptr: int, image_host_ptr: int, cuda_stream: int = 0) -> int:
     return load_library().pdm_migrate_host(plan, ctypes.c_void_p(P0_host_ptr),
                                            ctypes.c_void_p(image_host_ptr), ctypes.c_void_p(cuda_stream))
+
+
+def pdm_migrate_static(nx, nz, nw, dz, omega_dev_ptr: int, velocity_dev_ptr: int, table_dev_ptr: int,
+                       ntab, ntaps, tab_du, P0_dev_ptr: int, image_dev_ptr: int, cuda_stream: int = 0) -> int:
+    """Raw call of pdm.h's pdm_migrate_static: the migration for callers that may not allocate device
+    memory (every pointer is a DEVICE address the caller owns; scratch is the library's built-in 16 MiB
+    array, so nx*nw <= PDM_STATIC_MAX_SAMPLES).  Returns the status."""
+    vp = ctypes.c_void_p
+    return int(load_library().pdm_migrate_static(int(nx), int(nz), int(nw), float(dz), vp(omega_dev_ptr),
+                                                 vp(velocity_dev_ptr), vp(table_dev_ptr), int(ntab), int(ntaps),
+                                                 float(tab_du), vp(P0_dev_ptr), vp(image_dev_ptr), vp(cuda_stream)))
+
+
+def migrate_static(omega, velocity, table, dz, tab_du, P0, image, stream=None):
+    """pdm_migrate_static on torch CUDA tensors the caller already holds: omega float32 [nw], velocity
+    float32 [nz, nx], table complex64 [ntab, ntaps], P0 complex64 [nw, nx] -> image float32 [nz, nx]
+    (filled asynchronously, returned).  For code that must not trigger a device allocation: this
+    wrapper creates no tensor (hence `image` is required) and the library call allocates nothing.
+    All calls on one GPU share one scratch array -- keep them on one stream or order them with events."""
+    import torch
+    nz, nx = velocity.shape
+    nw = omega.shape[0]
+    ntab, ntaps = table.shape
+    want = ((omega, torch.float32, (nw,)), (velocity, torch.float32, (nz, nx)), (table, torch.complex64, (ntab, ntaps)),
+            (P0, torch.complex64, (nw, nx)), (image, torch.float32, (nz, nx)))
+    for t, dt, shape in want:
+        if not (t.is_cuda and t.dtype == dt and t.is_contiguous() and tuple(t.shape) == shape
+                and t.device == P0.device):
+            raise ValueError(f"expected a contiguous CUDA {dt} tensor of shape {shape} on {P0.device}")
+    st = (stream or torch.cuda.current_stream(P0.device)).cuda_stream
+    rc = pdm_migrate_static(nx, nz, nw, dz, omega.data_ptr(), velocity.data_ptr(), table.data_ptr(), ntab, ntaps,
+                            tab_du, P0.data_ptr(), image.data_ptr(), st)
+    if rc != PDM_OK:
+        raise PdmError(rc, "pdm_migrate_static")
+    return image
 
 
 def pdm_destroy(plan) -> int:

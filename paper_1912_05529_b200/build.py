@@ -18,6 +18,7 @@ OBJDIR = os.path.join(_HERE, "build")
 UNITS = [("pdm_api.cu", [], "pdm_api.o"),
          ("pdm_design.cu", [], "pdm_design.o"),
          ("pdm3_api.cu", [], "pdm3_api.o"),
+         ("pdm_static.cu", [], "pdm_static.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=0"], "tu_march0.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=1"], "tu_march1.o"),
          ("tu_march.cu", ["-DPDM_TU_PART=2"], "tu_march2.o"),

@@ -35,6 +35,7 @@ extern "C" const char *pdm_strerror(int code)
     case PDM_ERR_UNSUPPORTED: return "unsupported device, path or filter length";
     case PDM_ERR_NOMEM: return "out of memory";
     case PDM_ERR_CUDA: return "CUDA call failed (see pdm_info.last_cuda_error)";
+    case PDM_ERR_TOO_LARGE: return "nx*nw exceeds PDM_STATIC_MAX_SAMPLES (the built-in scratch of pdm_migrate_static)";
     default: return "unknown pdm_status";
     }
 }
