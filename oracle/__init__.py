@@ -6,3 +6,4 @@ import this package.  It imports nothing from the CUDA package and shares no cod
 from .oracle import build, migrate, migrate_field, migrate_shot, migrate3d, table_index, num_threads  # noqa: F401
 from .brute import brute_force_migrate  # noqa: F401
 from .tf_oracle import section_to_fx  # noqa: F401
+from . import design_oracle  # noqa: F401

@@ -129,11 +129,17 @@ def _table_du(omega: np.ndarray, dz: float, v_in: np.ndarray, ntab: int) -> floa
     return u_max / (ntab - 1)
 
 
+def _filters_source_hash() -> str:
+    """The cache key follows the SOURCE of the design: an edited filters.py never meets a stale table."""
+    with open(filters.__file__, "rb") as fh:
+        return hashlib.sha1(fh.read()).hexdigest()
+
+
 def cached_table(ntab: int, ntaps: int, du: float, r: float) -> np.ndarray:
     """Design (or fetch from the on-disk cache) the table for (ntab, ntaps, du, r)."""
     key = hashlib.sha1(repr((ntab, ntaps, float(du).hex(), float(r).hex(),
                              filters.NGRID, filters.PASSBAND_ANGLE_DEG, filters.STOP_CAP,
-                             "v1")).encode()).hexdigest()[:16]
+                             _filters_source_hash())).encode()).hexdigest()[:16]
     path = os.path.join(_CACHE_DIR, f"table_{ntaps}_{key}.npy")
     if os.path.exists(path):
         try:

@@ -54,9 +54,9 @@ def response_on_grid(half_taps: np.ndarray, ncheck: int = NCHECK) -> np.ndarray:
     return half @ cosm
 
 
-def design_table(ntab: int, ntaps: int, du: float, r: float = 1.0,
-                 n_iter: int = 200) -> np.ndarray:
-    """Design the full table: complex64 [ntab, ntaps], exactly symmetric, |H| <= 1 (D1-D4)."""
+def design_half_taps(ntab: int, ntaps: int, du: float, r: float = 1.0,
+                     n_iter: int = 200) -> np.ndarray:
+    """D1-D3 in FP64: complex128 [ntab, L+1] half taps W_0..W_L, normalised, before the cast."""
     if ntaps % 2 != 1 or ntaps < 1:
         raise ValueError("ntaps must be odd")
     L = (ntaps - 1) // 2
@@ -91,8 +91,14 @@ def design_table(ntab: int, ntaps: int, du: float, r: float = 1.0,
 
     # D3: normalise so that max |H| <= 1, then round to complex64 and re-check
     mag_max = np.abs(response_on_grid(half)).max(axis=1)
-    half = half / (np.maximum(mag_max, 1.0) * (1.0 + 4e-7))[:, None]
-    half32 = half.astype(np.complex64)
+    return half / (np.maximum(mag_max, 1.0) * (1.0 + 4e-7))[:, None]
+
+
+def design_table(ntab: int, ntaps: int, du: float, r: float = 1.0,
+                 n_iter: int = 200) -> np.ndarray:
+    """Design the full table: complex64 [ntab, ntaps], exactly symmetric, |H| <= 1 (D1-D4)."""
+    L = (ntaps - 1) // 2
+    half32 = design_half_taps(ntab, ntaps, du, r, n_iter).astype(np.complex64)
     table = np.empty((ntab, ntaps), dtype=np.complex64)
     table[:, L] = half32[:, 0]
     for k in range(1, L + 1):

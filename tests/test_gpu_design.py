@@ -1,6 +1,8 @@
 """Device-side extrapolator-table design (pdm_design_table)
-against the FP64 CPU statement of the same recipe D1-D4 (pdm_inputs/filters.py::design_table, which
-no product code imports and which pins P4/P6 already exercise on the oracle side).
+against the FP64 oracle of the recipe D1-D4, oracle/design_oracle.py: the literal full-grid FFT statement,
+pinned by tests/test_design_oracle_pins.py (G-P1..G-P4: DFT definition, a second statement of the recipe,
+the analytic phase shift on the passband).  The device kernel works on the half grid with cosine sums, so
+the two sides share no algebra; the analytic passband check is repeated here on the device-made table.
 
 Tolerance: both sides iterate in FP64 with different summation orders and cosine evaluations
 (relative differences ~1e-13 before the final rounding), so after rounding to complex64 the taps
@@ -13,6 +15,7 @@ import pytest
 
 import oracle
 import pdm_inputs
+from oracle import design_oracle
 from pdm_inputs import filters
 
 pytestmark = pytest.mark.gpu
@@ -29,9 +32,9 @@ def pdm():
 
 @pytest.mark.parametrize("ntab,ntaps,du,r", [(96, 15, 3.2 / 95, 1.0), (64, 25, 5.0 / 63, 1.0),
                                              (40, 51, 4.2 / 39, 1.0), (33, 9, 3.0 / 32, 0.5), (8, 1, 0.4, 1.0)])
-def test_device_design_matches_the_fp64_cpu_recipe(pdm, ntab, ntaps, du, r):
+def test_device_design_matches_the_fp64_oracle(pdm, ntab, ntaps, du, r):
     got = pdm.pdm_design_table(ntab, ntaps, du, r)
-    want = filters.design_table(ntab, ntaps, du, r)
+    want = design_oracle.design_table(ntab, ntaps, du, r)
     assert got.shape == want.shape and got.dtype == np.complex64
     L = (ntaps - 1) // 2
     # exact symmetry, bit for bit
@@ -42,8 +45,24 @@ def test_device_design_matches_the_fp64_cpu_recipe(pdm, ntab, ntaps, du, r):
     same = (got.view(np.uint64) == want.view(np.uint64)).mean()
     assert same >= 0.9, same
     # pin P6 on the DEVICE-made table: |H_j(kappa)| <= 1 + 1e-6 on 16384 points after rounding
-    H = filters.response_on_grid(got[:, L:], 16384)
-    assert np.abs(H).max() <= 1.0 + 1e-6
+    kap = np.pi * np.arange(16384) / 16383
+    assert np.abs(design_oracle.response(got.astype(np.complex128), kap)).max() <= 1.0 + 1e-6
+
+
+@pytest.mark.parametrize("ntaps,ntab,umax,bound_all,bound_mid", [(25, 48, 4.2, 3.5e-2, 2.0e-2), (51, 32, 4.2, 1.2e-2, 7.0e-3)])
+def test_device_designed_rows_are_the_one_way_phase_shift_on_the_passband(pdm, ntaps, ntab, umax, bound_all, bound_mid):
+    """Independent of D1-D4's code on either side: |H_j(kappa) - exp(+i sqrt(u_j^2 - kappa^2))| on random
+    passband kappa, bounds as pin G-P3 (plus the complex64 rounding, < 1e-5)."""
+    rng = np.random.default_rng(ntaps + 1)
+    du = umax / (ntab - 1)
+    got = pdm.pdm_design_table(ntab, ntaps, du, 1.0).astype(np.complex128)
+    for j in range(1, ntab):
+        u = j * du
+        edge = min(u * np.sin(np.deg2rad(55.0)), 0.8 * np.pi)
+        kap = rng.uniform(-edge, edge, 400)
+        exact = np.exp(1j * np.sqrt(u * u - kap * kap))
+        err = np.abs(design_oracle.response(got[j], kap) - exact).max()
+        assert err <= (bound_mid if u >= 0.6 else bound_all) + 1e-5, (j, u, err)
 
 
 def test_device_design_options_and_errors(pdm):
