@@ -66,7 +66,14 @@ typedef enum {
 #define PDM_PATH_PACKED  5u  /* x-tiled AND temporally blocked (T depth steps per tile visit, planes   */
                              /* cross HBM once per T steps, tiles moved by TMA) with 8 adjacent       */
                              /* frequencies per quarter warp, which makes the per-sample tap gather   */
-                             /* bank-conflict free; any nx                        */
+                             /* bank-conflict free; any nx.  Tap rows are staged  */
+                             /* per tile visit in shared memory; where one pack's row range on a     */
+                             /* visit is wider than any slice buffer (velocity varying > ~2x inside  */
+                             /* a tile at the top frequencies with 51 taps and 1024 rows) forced,    */
+                             /* PDM_PRESTACK and PDM_TAPER plans read the rows from the global table */
+                             /* instead (256-thread build, pdm_info.taps_mode = 1; slower, same      */
+                             /* bits); AUTO poststack plans take another form.  A forced CTA size of */
+                             /* 384 or 512 threads then gives PDM_ERR_UNSUPPORTED                    */
 #define PDM_PATH_MASK    0xFu
 #define PDM_TAPS_AUTO    (0u << 4)  /* where the kernels read filter rows from                      */
 #define PDM_TAPS_GLOBAL  (1u << 4)  /* always from the L2/L1-cached global half-table               */

@@ -89,7 +89,12 @@ __device__ __forceinline__ void pdm_tma_load_2d(unsigned dst, const CUtensorMap 
 }
 
 // NTHREADS = CTA size the instantiation is compiled for (512: 128 registers per thread; 384: 168; 256: 255)
-template <int L, bool SYM, int NTHREADS>
+// GTAPS = true: tap rows are never staged; every fetch reads the global half table (L1/L2).  The plan
+// takes this build (256 threads only) when one pack's row range on some tile visit is wider than any
+// slice buffer -- strongly varying velocity inside a tile at the top frequencies, e.g. a salt flank or
+// a model with independent samples and a 1024-row table -- so that PDM_PRESTACK / PDM_TAPER / forced
+// PDM_PATH_PACKED plans exist for ANY table and model ("filter cutoffs may vary for each point").
+template <int L, bool SYM, int NTHREADS, bool GTAPS = false>
 __global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_constant__ pdm_pack_params p)
 {
     constexpr int R = 8, W = PDM_PACK_W;
@@ -183,7 +188,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_cons
 
         for (int k = 0; k < nmine; ++k) {
             const bool new_tile = tile != cur_tile;
-            const bool restage = tile != st_tile || blk != st_blk || pack > st_hi || pack < st_lo;
+            const bool restage = !GTAPS && (tile != st_tile || blk != st_blk || pack > st_hi || pack < st_lo);
             if (new_tile || restage) {                                    // CTA-uniform, rare
                 __syncthreads();                                          // every warp is done with the old slice / tile
                 if (new_tile) {
@@ -266,12 +271,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) pdm_pack_kernel(const __grid_cons
                     const int soff = l * p.LS + R * HG + R * g + 2 * l;
                     const float2 *base = cur + soff;
                     float2 out[R];
+                    const float4 *const tb = GTAPS ? p.half : slice;    // jlo stays 0 with GTAPS: global row offsets
                     if (SYM) {
-                        if (uni) pdm_fir_group<L, R, true, false, 0u, 0>(base, slice, toff, out);
-                        else     pdm_fir_group<L, R, false, false, 0u, 0>(base, slice, toff, out);
+                        if (uni) pdm_fir_group<L, R, true, false, 0u, 0>(base, tb, toff, out);
+                        else     pdm_fir_group<L, R, false, false, 0u, 0>(base, tb, toff, out);
                     } else {
-                        if (uni) pdm_fir_group_asym<L, R, true, 0>(base, slice, toff, out);
-                        else     pdm_fir_group_asym<L, R, false, 0>(base, slice, toff, out);
+                        if (uni) pdm_fir_group_asym<L, R, true, 0>(base, tb, toff, out);
+                        else     pdm_fir_group_asym<L, R, false, 0>(base, tb, toff, out);
                     }
                     if (xg < 0 || xg + R > p.nx) {                      // R5: zero outside [0,nx) (edge groups only)
 #pragma unroll

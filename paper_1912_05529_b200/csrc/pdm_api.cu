@@ -201,9 +201,9 @@ static tiled_fn tiled_kernel_for(const pdm_plan *p, bool wide)
 }
 static pack_fn pack_kernel_for(const pdm_plan *p)
 {
-    pack_fn f = pdm_pack_kernel_part0(p->Lk, p->sym != 0, p->threads);
-    if (!f) f = pdm_pack_kernel_part1(p->Lk, p->sym != 0, p->threads);
-    if (!f) f = pdm_pack_kernel_part2(p->Lk, p->sym != 0, p->threads);
+    pack_fn f = pdm_pack_kernel_part0(p->Lk, p->sym != 0, p->threads, p->pk_gtaps != 0);
+    if (!f) f = pdm_pack_kernel_part1(p->Lk, p->sym != 0, p->threads, p->pk_gtaps != 0);
+    if (!f) f = pdm_pack_kernel_part2(p->Lk, p->sym != 0, p->threads, p->pk_gtaps != 0);
     return f;
 }
 // TMA descriptor of a [nrows][row_samples] array of 8-byte samples (complex64 moved as opaque 64-bit
@@ -213,7 +213,7 @@ typedef CUresult (*pdm_encode_fn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
                                   CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
                                   CUtensorMapFloatOOBfill);
-static int make_plane_map(pdm_plan *p, CUtensorMap *map, const void *base, int row_samples, int nrows, int box)
+static pdm_encode_fn tensor_map_encoder()
 {
     static pdm_encode_fn enc = nullptr;
     if (!enc) {
@@ -222,10 +222,16 @@ static int make_plane_map(pdm_plan *p, CUtensorMap *map, const void *base, int r
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &sym, cudaEnableDefault, &qr) != cudaSuccess ||
             qr != cudaDriverEntryPointSuccess || !sym) {
             cudaGetLastError();
-            return PDM_ERR_UNSUPPORTED;
+            return nullptr;
         }
         enc = (pdm_encode_fn)sym;
     }
+    return enc;
+}
+static int make_plane_map(pdm_plan *p, CUtensorMap *map, const void *base, int row_samples, int nrows, int box)
+{
+    const pdm_encode_fn enc = tensor_map_encoder();
+    if (!enc) return PDM_ERR_UNSUPPORTED;
     const cuuint64_t dims[2] = { (cuuint64_t)row_samples, (cuuint64_t)nrows };
     const cuuint64_t strides[1] = { (cuuint64_t)row_samples * sizeof(float2) };
     const cuuint32_t boxd[2] = { (cuuint32_t)box, 1u }, estr[2] = { 1u, 1u };
@@ -314,8 +320,11 @@ static int build_packed(pdm_plan *p, const float *omega, const std::vector<float
 {
     const int nx = p->nx, nz = p->nz, nw = p->nw, ntab = p->ntab, R = PDM_R;
     int rc;
+    // the TMA descriptor encoder is part of feasibility: without it AUTO must fall back with nothing allocated
+    if (!tensor_map_encoder()) return PDM_ERR_UNSUPPORTED;
     // kern_pack.cuh: 8 adjacent frequencies per quarter warp, T depth steps per tile visit
     p->taps_mode = 2;
+    p->pk_gtaps = 0;
     const int W = PDM_PACK_W;
     // the tuning bits mean something else for the other forms: read them only when this form is forced
     const bool forced = (p->flags & PDM_PATH_MASK) == PDM_PATH_PACKED;
@@ -338,7 +347,11 @@ static int build_packed(pdm_plan *p, const float *omega, const std::vector<float
     const int nblocks = (nz + T - 1) / T;
     std::vector<float2> tileq;
     size_t fixed = 0;
-    for (int cand = 512; cand >= 256 && !NT; cand -= 128) {
+    // Plans that have no other form to fall back to (forced, prestack, taper) get a second round: the
+    // 256-thread build that reads tap rows from the global table, for which no row range is too wide.
+    const bool must_exist = forced || p->prestack || p->ntaper > 0;
+    for (int round = 0; round < (must_exist ? 2 : 1) && !NT; ++round)
+    for (int cand = round ? 256 : 512; cand >= 256 && !NT; cand -= 128) {
         if (nsel && cand != 32 * (int)nsel) continue;
         passes = cand == 256 ? 2 : 1;                  // groups per thread and step
         TXH = cand / W * R * passes;                   // samples a CTA computes per line and step
@@ -371,9 +384,15 @@ static int build_packed(pdm_plan *p, const float *omega, const std::vector<float
         fixed = 128 + lines_bytes + img_bytes;
         const size_t budget = (size_t)p->smem_optin - 1024;   // the kernel's static shared memory counts too
         if (fixed >= budget) continue;
-        cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
-        if (cap < maxrows) continue;                   // one pack's rows must fit next to the line tiles
-        cap = std::min(cap, ntab);
+        if (round) {                                   // global tap rows: no slice buffer at all
+            cap = 0;
+            p->pk_gtaps = 1;
+            p->taps_mode = 1;
+        } else {
+            cap = (int)((budget - fixed) / ((size_t)p->half16 * sizeof(float4)));
+            if (cap < maxrows) continue;               // one pack's rows must fit next to the line tiles
+            cap = std::min(cap, ntab);
+        }
         NT = cand;
     }
     if (!NT) return PDM_ERR_UNSUPPORTED;

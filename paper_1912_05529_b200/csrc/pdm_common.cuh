@@ -62,6 +62,7 @@ struct pdm_plan {
     int taps_in_smem;     // march: 1 = per-omega rows staged in shared memory, 0 = L1/L2 global rows
     // packed path (kern_pack.cuh): planes [nw][nxp] ping-pong, T depth steps per tile visit
     int nxp, pk_T, pk_TX, pk_H, pk_LS, pk_BW, pk_nbox, pk_cap, pk_passes, pk_npacks, pk_ntiles;
+    int pk_gtaps;         // 1: tap rows read from the global table (a pack's row range exceeds every slice buffer)
     float2 *d_packw;      // [npacks] lowest / highest omega of a pack
     float2 *d_tileq;      // [nblocks][ntiles] min / max q over the samples a tile visit computes
     int2 *d_tile_ctas;    // [ntiles] first / last CTA that holds a piece of the tile's image

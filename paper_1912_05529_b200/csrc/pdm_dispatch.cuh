@@ -40,6 +40,6 @@ tiled_fn   pdm_tiled_kernel_asym_part0(int L, bool wide);
 tiled_fn   pdm_tiled_kernel_asym_part1(int L, bool wide);
 tiled_fn   pdm_tiled_kernel_asym_part2(int L, bool wide);
 // frequency-packed, temporally blocked x-tiled form (tu_pack.cu, same three parts)
-pack_fn    pdm_pack_kernel_part0(int L, bool sym, int threads);
-pack_fn    pdm_pack_kernel_part1(int L, bool sym, int threads);
-pack_fn    pdm_pack_kernel_part2(int L, bool sym, int threads);
+pack_fn    pdm_pack_kernel_part0(int L, bool sym, int threads, bool gtaps);
+pack_fn    pdm_pack_kernel_part1(int L, bool sym, int threads, bool gtaps);
+pack_fn    pdm_pack_kernel_part2(int L, bool sym, int threads, bool gtaps);

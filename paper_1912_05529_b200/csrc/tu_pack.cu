@@ -24,7 +24,19 @@ static pack_fn pick(int L, bool sym)
     }
 }
 
-pack_fn PDM_PART_FN(int L, bool sym, int threads)
+// the build that reads tap rows from the global table (256 threads only; see kern_pack.cuh)
+static pack_fn pick_gtaps(int L, bool sym)
 {
+    switch (L) {
+#define X(LL) case LL: return sym ? pdm_pack_kernel<LL, true, 256, true> : pdm_pack_kernel<LL, false, 256, true>;
+        PDM_L_THIS(X)
+#undef X
+    default: return nullptr;
+    }
+}
+
+pack_fn PDM_PART_FN(int L, bool sym, int threads, bool gtaps)
+{
+    if (gtaps) return threads == 256 ? pick_gtaps(L, sym) : nullptr;
     return threads == 256 ? pick<256>(L, sym) : threads == 384 ? pick<384>(L, sym) : threads == 512 ? pick<512>(L, sym) : nullptr;
 }

@@ -228,6 +228,51 @@ def test_edge_taper_variant_matches_oracle(pdm, model, nx, nz, nw, ntaps, n, T):
         assert rc == pdm.PDM_ERR_INVALID_ARG and h is None
 
 
+@pytest.mark.parametrize("sym", [True, False])
+def test_packed_form_with_row_ranges_wider_than_any_slice_buffer(pdm, sym):
+    """51 taps, ntab = 1024, independent samples with a 3.3x velocity spread: at the top frequencies one
+    pack's rows on a tile visit span ~700 table rows, more than the ~518 the shared-memory slice holds.
+    Forced PDM_PATH_PACKED and PDM_TAPER plans then run the build that reads tap rows from the global
+    table (pdm_info.taps_mode = 1) instead of failing; AUTO poststack takes another form."""
+    cfg = pdm_inputs.random_problem(61, 1100, 7, 19, 51, ntab=1024, model="white", symmetric=sym)
+    ref = oracle.migrate(cfg)
+    img, info = gpu_migrate(pdm, cfg, pdm.PDM_PATH_PACKED, want_info=True)
+    assert info["path"] == pdm.PDM_PATH_PACKED and info["taps_mode"] == 1 and info["threads_per_cta"] == 256, info
+    rel, mx = errors(img, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info)
+    img2, info2 = gpu_migrate(pdm, cfg, pdm.PDM_PATH_PACKED | (3 << pdm.PDM_CTAS_SHIFT) | pdm.PDM_FORCE_GENERAL, want_info=True)
+    assert info2["taps_mode"] == 1
+    rel, mx = errors(img2, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info2)
+    n = 30
+    timg, tinfo = gpu_migrate(pdm, cfg, n << pdm.PDM_TAPER_SHIFT, want_info=True)
+    assert tinfo["path"] == pdm.PDM_PATH_PACKED and tinfo["taps_mode"] == 1, tinfo
+    rel, mx = errors(timg, oracle.migrate(cfg, ntaper=n))
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, tinfo)
+    _, auto = gpu_migrate(pdm, cfg, 0, want_info=True)              # AUTO still plans (any form), staged or not
+    assert auto["path"] != pdm.PDM_PATH_NAIVE
+    args = (cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"], cfg["velocity"], cfg["table"], cfg["du"])
+    rc, h = pdm.pdm_create(*args, pdm.PDM_PATH_PACKED | (16 << pdm.PDM_THREADS_SHIFT))   # the global-row build is 256 threads only
+    assert rc == pdm.PDM_ERR_UNSUPPORTED and h is None
+
+
+@pytest.mark.parametrize("sym,T,n", [(True, 1, 0), (True, 4, 25), (False, 4, 0), (False, 1, 25), (True, 0, 0)])
+def test_packed_form_many_items_per_cta(pdm, sym, T, n):
+    """nitems = tiles x packs far above the 148-CTA grid (here ~45 x 8 = 360): every CTA runs several
+    items per depth block, so the double-buffered TMA refill (issue(k+2) by the last warp), the mbarrier
+    parities across items and blocks, slice reuse over packs, the image flush on a tile change and the
+    progress flags carried across items all run -- with asymmetric tables, the taper and forced T."""
+    cfg = pdm_inputs.random_problem(67, 20011, 6, 61, 7, model="field", symmetric=sym)
+    flags = pdm.PDM_PATH_PACKED | (T << pdm.PDM_CTAS_SHIFT) | (n << pdm.PDM_TAPER_SHIFT)
+    img, info = gpu_migrate(pdm, cfg, flags, want_info=True)
+    assert info["path"] == pdm.PDM_PATH_PACKED and info["grid_ctas"] <= info["sm_count"], info
+    ref = oracle.migrate(cfg, ntaper=n)
+    rel, mx = errors(img, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx, info)
+    again = gpu_migrate(pdm, cfg, flags)
+    assert np.array_equal(img, again)
+
+
 def test_packed_path_with_unaligned_p0_pointer(pdm):
     """Even nx but a P0 that is only 8-byte aligned: TMA cannot address it, so the library repacks it
     into its own plane first; same image bit for bit as the direct descriptor on an aligned P0."""

@@ -59,6 +59,40 @@ def test_shot_matches_oracle(pdm, T, model, nx, nz, nw, ntaps, sym):
         assert pdm.pdm_migrate(plan._h, r.data_ptr(), a.data_ptr(), 0) == pdm.PDM_ERR_INVALID_ARG
 
 
+def test_shot_with_row_ranges_wider_than_any_slice_buffer(pdm):
+    """Prestack plans have no other kernel form to fall back to: with 51 taps, 1024 table rows and
+    independent samples (row range of a pack ~700 > the ~518 rows a slice holds) the plan must still
+    exist -- on the build that reads tap rows from the global table."""
+    import torch
+    nx, nz, nw = 1100, 6, 9
+    cfg = pdm_inputs.random_problem(71, nx, nz, nw, 51, ntab=1024, model="white")
+    S0, R0 = _fields(np.random.default_rng(3), nw, nx)
+    ref = oracle.migrate_shot(cfg, S0, R0)
+    with pdm.Plan.from_config(cfg, pdm.PDM_PRESTACK) as plan:
+        info = plan.info
+        assert info["path"] == pdm.PDM_PATH_PACKED and info["taps_mode"] == 1, info
+        a = plan.migrate_shot(torch.from_numpy(S0).cuda(), torch.from_numpy(R0).cuda())
+        torch.cuda.synchronize()
+        rel, mx = _errors(a.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx, info)
+
+
+@pytest.mark.parametrize("sym,T", [(True, 1), (False, 4)])
+def test_shot_many_items_per_cta(pdm, sym, T):
+    """~45 tiles x 8 packs on 148 CTAs: several items per CTA and depth block in the cross-correlation mode."""
+    import torch
+    nx, nz, nw = 20011, 5, 31
+    cfg = pdm_inputs.random_problem(73, nx, nz, nw, 7, model="field", symmetric=sym)
+    S0, R0 = _fields(np.random.default_rng(5), nw, nx)
+    ref = oracle.migrate_shot(cfg, S0, R0)
+    with pdm.Plan.from_config(cfg, pdm.PDM_PRESTACK | pdm.PDM_PATH_PACKED | (T << pdm.PDM_CTAS_SHIFT)) as plan:
+        info = plan.info
+        a = plan.migrate_shot(torch.from_numpy(S0).cuda(), torch.from_numpy(R0).cuda())
+        torch.cuda.synchronize()
+        rel, mx = _errors(a.cpu().numpy(), ref)
+    assert rel <= 1e-4 and mx <= 1e-3, (rel, mx, info)
+
+
 def test_shots_accumulate_into_one_image(pdm):
     import torch
     cfg = pdm_inputs.random_problem(59, 900, 14, 12, 25, model="field")
