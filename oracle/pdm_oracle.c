@@ -168,7 +168,13 @@ int pdm_oracle_migrate_taper(int nx, int nz, int nw, double dz,
         if (!P || !Pn) {
 #pragma omp atomic write
             failed = 1;
-        } else {
+        }
+        /* every thread must reach the work-sharing loop or none: decide together after a barrier */
+        int any_failed;
+#pragma omp barrier
+#pragma omp atomic read
+        any_failed = failed;
+        if (!any_failed) {
 #pragma omp for schedule(static)
             for (int il = 0; il < nlines; ++il) {                       /* O2 */
                 const int iw = nsub > 0 ? omega_index[il] : il;
@@ -340,7 +346,13 @@ int pdm_oracle_migrate3d(int nx, int ny, int nz, int nw, double dz,
         if (!P || !Pn) {
 #pragma omp atomic write
             failed = 1;
-        } else {
+        }
+        /* every thread must reach the work-sharing loop or none: decide together after a barrier */
+        int any_failed;
+#pragma omp barrier
+#pragma omp atomic read
+        any_failed = failed;
+        if (!any_failed) {
 #pragma omp for schedule(static)
             for (int iw = 0; iw < nw; ++iw) {
                 const float w32 = omega[iw];
