@@ -550,6 +550,35 @@ def test_config4_more_points_sampled_frequencies(pdm, nx, nw, ntaps, model, flag
     _subset_parity(pdm, cfg, _sample_lines(info, nw), flags)
 
 
+# The other 28 points of the 48-point field sweep ("for the remaining points verify parity on a
+# seeded omega-subset"), each with the kernel form AUTO chose when profiles/r02_sweep_config4.md section 1 was
+# measured: S = SMEM marching, C = cluster, T = x-tiled, P = frequency-packed.
+CONFIG4_REST = [
+    (1024, 256, 15, "S"), (1024, 1024, 15, "S"), (4096, 64, 15, "C"), (4096, 1024, 15, "P"),
+    (4096, 2048, 15, "P"), (16384, 256, 15, "C"), (16384, 2048, 15, "P"), (32768, 256, 15, "P"),
+    (32768, 1024, 15, "P"), (1024, 256, 25, "S"), (1024, 1024, 25, "S"), (4096, 64, 25, "C"),
+    (4096, 1024, 25, "P"), (4096, 2048, 25, "P"), (16384, 64, 25, "T"), (16384, 256, 25, "P"),
+    (16384, 2048, 25, "P"), (32768, 1024, 25, "P"), (1024, 256, 51, "S"), (1024, 1024, 51, "S"),
+    (4096, 64, 51, "C"), (4096, 1024, 51, "P"), (4096, 2048, 51, "P"), (16384, 64, 51, "T"),
+    (16384, 256, 51, "P"), (16384, 2048, 51, "P"), (32768, 256, 51, "P"), (32768, 1024, 51, "P"),
+]
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("nx,nw,ntaps,form", CONFIG4_REST)
+def test_config4_remaining_points_sampled_frequencies(pdm, nx, nw, ntaps, form):
+    """Full size, AUTO launch configuration (what bench.py --sweep times): >= 8 sampled frequency lines
+    (first / last, CTA work-range boundaries) against the oracle, and the path the sweep table reports."""
+    cfg = pdm_inputs.sweep_point(nx, nw, ntaps)
+    with pdm.Plan.from_config(cfg, 0) as plan:
+        info = plan.info
+    want = {"S": pdm.PDM_PATH_SMEM, "C": pdm.PDM_PATH_CLUSTER, "T": pdm.PDM_PATH_TILED, "P": pdm.PDM_PATH_PACKED}[form]
+    assert info["path"] == want, info
+    lines = _sample_lines(info, nw, want=8)[:12]
+    assert len(lines) >= 8
+    _subset_parity(pdm, cfg, lines, 0, expect_path=want)
+
+
 @pytest.mark.slow
 def test_randomized_parity_over_forms_shapes_and_filter_lengths(pdm):
     """Seeded fuzz: random (nx, nz, nw, taps, model, kernel form) -- ragged sizes around the 8-sample
