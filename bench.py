@@ -97,6 +97,20 @@ def workload_name(k: int, cfg: dict, world: int) -> str:
     return s
 
 
+def bench_config(k: int, cfg: dict, world: int) -> dict:
+    """The `config` object, identical in both arms (launch details of our arm go under `launch`)."""
+    return {"workload": workload_name(k, cfg, world),
+            "l2": "GPU arm: 256 MiB buffer written between timed steps (L2 flush), CUDA events on the launching "
+                  "stream; reference arm: the FP64 oracle on the host cores, wall clock"}
+
+
+def executed_frac(info: dict, seconds: float) -> float:
+    """FP32 lane-operations the kernels actually execute (pdm_info.executed_lane_ops: folded taps counted
+    once, zero-padded taps counted) x 2 flop / time / the derived FP32 peak -- beside the COUNTED fraction,
+    whose ratio to this one differs per kernel family (1.32 folded 1-D, 1.0 general, 2.45 folded 15x15 3-D)."""
+    return info["executed_lane_ops"] * 2.0 / seconds / (FP32_PEAK_NOMINAL_TFLOPS * 1e12)
+
+
 # ------------------------------------------------------------------------------- clocks
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
@@ -172,11 +186,13 @@ def run_reference(args, rank: int, world: int):
         return
     cfg = load_workload(args.config, 0, 1)
     import oracle
-    # size the per-step sample so warmup+steps stay within a few minutes: ~1 line per thread
+    # per-step sample: 4 lines per thread (the cpu_baseline leg of our arm takes 16, once): large enough that
+    # the oracle's fixed costs (q map, per-thread image accumulators) no longer depress the rate, small
+    # enough that warmup + steps stay within a few minutes at configs[3] (~3 s per step on 16 cores)
     threads = oracle.num_threads()
     times, sps = [], []
     for i in range(args.warmup + args.steps):
-        v, dt, nlines, threads = oracle_sample(cfg, lines_per_thread=1)
+        v, dt, nlines, threads = oracle_sample(cfg, lines_per_thread=args.ref_lines_per_thread)
         if i >= args.warmup:
             times.append(dt); sps.append(v)
     value = float(np.mean(sps))
@@ -185,7 +201,7 @@ def run_reference(args, rank: int, world: int):
     out = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * float(np.mean(times)),
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-           "data": "synthetic", "config": {"workload": workload_name(args.config, cfg, 1)},
+           "data": "synthetic", "config": bench_config(args.config, cfg, 1),
            "cpu_baseline": {"value": value, "unit": UNIT, "cores": threads, "kind": "oracle",
                             "sample": sample},
            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -254,6 +270,7 @@ def other_configs(pdm, torch, dev, stream, flush):
                      "path": PATH_NAMES[info["path"]], "ms_median": t * 1e3, "ms_best": float(min(ms)),
                      "samples_per_s": sps,
                      "frac_fp32_peak_counted": sps * 8 * cfg["ntaps"] / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                     "frac_fp32_peak_executed": executed_frac(info, t),
                      "frac_hbm_16B_per_sample_of_measured":
                          (sps * 16 / (measured_hbm_gbs()[0] * 1e9)) if info["path"] == pdm.PDM_PATH_TILED else None})
         if name in ("configs[0]", "configs[1]"):
@@ -383,6 +400,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
         roofline = {"bound": "alu", "kernel": kernel, "achieved": achieved,
                     "peak": FP32_PEAK_NOMINAL_TFLOPS, "unit": "TFLOP/s",
                     "frac": achieved / FP32_PEAK_NOMINAL_TFLOPS,
+                    "frac_executed": executed_frac(info, main_avg * 1e-3),
                     "traffic": traffic,
                     "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum)",
                     "traffic_source": traffic_src,
@@ -404,12 +422,9 @@ def run_ours(args, rank: int, local_rank: int, world: int):
                "ms_per_step_median": float(np.median(step_ms)), "ms_per_step_best": float(min(step_ms)),
                "create_ms": create_ms, "higher_is_better": True,
                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-               "config": {"workload": workload_name(args.config, cfg, world),
-                          "path": path_name,
-                          "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
-                          "smem_bytes": info["smem_bytes"],
-                          "l2": "256 MiB buffer written between timed steps (L2 flush); plan workspace "
-                                f"{info['workspace_bytes'] / 1e9:.3f} GB"},
+               "config": bench_config(args.config, cfg, world),
+               "launch": {"path": path_name, "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
+                          "smem_bytes": info["smem_bytes"], "workspace_gb": info["workspace_bytes"] / 1e9},
                "pct_fp32_peak_counted": 100.0 * value / world * 8 * cfg["ntaps"] / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
                "roofline": roofline,
                "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cpu_threads, "kind": "oracle",
@@ -427,7 +442,7 @@ def run_ours(args, rank: int, local_rank: int, world: int):
             a2.flags, a2.steps = 0, min(args.steps, 5)
             out["extra"] = {"other_configs": other_configs(pdm, torch, dev, stream, flush),
                             # the stages around / beyond the poststack hot path, same run
-                            "other_stages": measure_tf(a2) + measure_prestack(a2) + measure_3d(a2)}
+                            "other_stages": measure_tf(a2) + measure_design(a2) + measure_prestack(a2) + measure_3d(a2)}
         print(json.dumps(out), flush=True)
     plan.close()
     if world > 1:
@@ -503,6 +518,7 @@ def run_sweep(args):
                        "launches": info["launches_per_migrate"], "steps": steps, "ms": t * 1e3,
                        "samples_per_s": sps,
                        "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                       "frac_fp32_peak_executed": executed_frac(info, t),
                        "frac_hbm_16B_per_sample": (sps * 16 / (hbm_gbs * 1e9)) if tiled else None,
                        "hbm_peak_gbs": hbm_gbs, "hbm_peak_source": hbm_src}
                 print(json.dumps(out), flush=True)
@@ -560,6 +576,33 @@ def measure_tf(args):
                       "share_of_migration": "compare ms with bench.py's ms_per_step on configs[3]"})]
 
 
+# ------------------------------------------------------------------------------- table design
+def measure_design(args):
+    """pdm_design_table for configs[3]'s table (1024 rows x 51 taps, 200 D2 sweeps on a
+    2048-point grid, FP64) -- a synchronous setup call, so wall clock around it (median of 3 after one warm-up)."""
+    import torch
+
+    import paper_1912_05529_b200 as pdm
+
+    pdm.load_library()
+    torch.cuda.set_device(0)
+    ntab, ntaps, du = 1024, 51, 4.19 / 1023
+    pdm.pdm_design_table(16, ntaps, du, 1.0)
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(3):
+        t0 = time.perf_counter()
+        pdm.pdm_design_table(ntab, ntaps, du, 1.0)
+        ts.append(time.perf_counter() - t0)
+    t = float(np.median(ts))
+    # per row and sweep: forward (N/2+1) x (L+1) + inverse (L+1) x (N/2+1) FP64 multiply-adds on the half grid
+    fma = 2.0 * 200 * ntab * (1024 + 1) * 26
+    return [{"workload": f"table design ntab={ntab} taps={ntaps} (configs[3]'s table), 200 sweeps, grid 2048, FP64",
+             "kernel": "pdm_design_kernel", "steps": 3, "ms": t * 1e3, "ms_best": float(min(ts)) * 1e3,
+             "rows_per_s": ntab / t, "fp64_tflops": 2.0 * fma / t / 1e12,
+             "includes": "host validation, cosine-table upload, kernel, D2H copy of the table (synchronous call)"}]
+
+
 # ------------------------------------------------------------------------------- prestack shot
 def measure_prestack(args):
     """one prestack shot (pdm_migrate_shot) on a configs[4] field point -- both
@@ -601,7 +644,8 @@ def measure_prestack(args):
                                   "(2 wavefields per frequency)", "kernel": "pdm_pack_kernel (xcorr)",
                       "path": PATH_NAMES[info["path"]], "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                       "steps": args.steps, "ms": t * 1e3, "ms_best": float(min(ms)), "samples_per_s": sps,
-                      "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12)})]
+                      "frac_fp32_peak_counted": sps * 8 * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                      "frac_fp32_peak_executed": executed_frac(info, t)})]
 
 
 # ------------------------------------------------------------------------------- 3-D variant
@@ -651,6 +695,7 @@ def measure_3d(args):
                               "smem_bytes": info["smem_bytes"], "steps": args.steps, "ms": t * 1e3,
                               "ms_best": float(min(ms)), "samples_per_s": sps,
                               "frac_fp32_peak_counted": sps * 8 * ntaps * ntaps / (FP32_PEAK_NOMINAL_TFLOPS * 1e12),
+                              "frac_fp32_peak_executed": executed_frac(info, t),
                               "frac_hbm_16B_per_sample": sps * 16 / (hbm_gbs * 1e9)}))
     return rows
 
@@ -679,6 +724,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[0, 1, 2, 3])
     ap.add_argument("--flags", type=lambda s: int(s, 0), default=0, help="pdm_create flags word")
     ap.add_argument("--cpu-lines-per-thread", type=int, default=16)
+    ap.add_argument("--ref-lines-per-thread", type=int, default=4,
+                    help="--impl reference: omega lines per host thread and step")
     ap.add_argument("--no-extra", action="store_true",
                     help="skip extra.other_configs (configs[0..2] + two configs[4] points, N = 1 only)")
     ap.add_argument("--tf", action="store_true", help="time the t->f transform of the section (SURVEY 8(f) N1)")
