@@ -44,7 +44,10 @@ typedef enum {
                                       with more than 51 taps (the longest unrolled kernel; shorter
                                       filters of any odd length run on the next longer kernel with
                                       zero taps appended, longer ones only on PDM_PATH_NAIVE)      */
-    PDM_ERR_NOMEM = -5,            /* host or device allocation failed                             */
+    PDM_ERR_NOMEM = -5,            /* host or device allocation failed.  pdm_create compares every large
+                                      request with the free device memory BEFORE allocating; the main
+                                      form needs grid_ctas*nz*nx*4 B of per-CTA partial images (the
+                                      total is pdm_info.workspace_bytes of a plan that was created)  */
     PDM_ERR_CUDA = -6,             /* a CUDA call failed; pdm_info.last_cuda_error has the code    */
     PDM_ERR_TOO_LARGE = -7         /* pdm_migrate_static only: nx*nw exceeds PDM_STATIC_MAX_SAMPLES, the
                                       size of the library's built-in scratch                       */
@@ -150,7 +153,9 @@ int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, float dz,
  *   cuda_stream  cudaStream_t (0 = legacy default stream).
  * Asynchronous on the stream; performs no allocation, no host synchronisation and no host<->device
  * copy (CUDA-graph capturable); bit-identical images on repeated calls (fixed summation order, no
- * float atomics).  One migrate in flight per plan (the workspace is per plan).
+ * float atomics).  One migrate in flight per plan (the workspace is per plan).  "Enqueue only" on the
+ * PDM_PATH_PACKED form includes one host-side encode of the TMA descriptor of the caller's P0 (a pure
+ * CPU computation of ~1 us, no driver state touched), because P0's address is only known at the call.
  * Errors: PDM_ERR_INVALID_ARG (NULL), PDM_ERR_CUDA (launch failure, wrong current device).
  */
 int pdm_migrate(pdm_plan *plan, const pdm_c64 *P0_dev, float *image_dev, void *cuda_stream);

@@ -71,6 +71,15 @@ static int dev_alloc(pdm_plan *p, T **ptr, size_t count)
 {
     *ptr = nullptr;
     if (count == 0) count = 1;
+    // Large requests (the per-CTA partial images of the marching form are grid*nz*nx*4 B: 5.5 GB for
+    // configs[3], 39 GB for a 16384 x 4000 image) are checked against the free memory first, so that a plan
+    // that cannot fit fails with PDM_ERR_NOMEM at once instead of after the driver has tried to make room.
+    if (count * sizeof(T) >= ((size_t)256 << 20)) {
+        size_t free_b = 0, total_b = 0;
+        if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+            if (count * sizeof(T) > free_b) { p->last_cuda_error = (int)cudaErrorMemoryAllocation; return PDM_ERR_NOMEM; }
+        } else cudaGetLastError();
+    }
     PDM_CUDA(p, cudaMalloc((void **)ptr, count * sizeof(T)));
     p->workspace_bytes += (double)(count * sizeof(T));
     return PDM_OK;

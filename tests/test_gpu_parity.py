@@ -608,6 +608,27 @@ def test_randomized_parity_over_forms_shapes_and_filter_lengths(pdm):
 
 
 # ---------------------------------------------------------------- properties of the GPU path itself
+def test_plan_that_cannot_fit_fails_with_nomem_and_leaks_nothing(pdm):
+    """The main form keeps one partial image per CTA (grid*nz*nx*4 B).  A plan whose partial images exceed
+    the free device memory must fail with PDM_ERR_NOMEM (checked before the allocation is attempted) and
+    give back everything it had allocated by then."""
+    import torch
+    nx, nz, nw = 4096, 90000, 160                       # 148 CTAs x 90000 x 4096 x 4 B = 218 GB
+    cfg = pdm_inputs.tiny_random_problem(3, nx=64, nz=2, nw=2, L=3, ntab=64)
+    omega = np.linspace(20.0, 60.0, nw).astype(np.float32)
+    vel = np.full((nz, nx), 2000.0, dtype=np.float32)
+    du = float(omega.max()) * 10.0 / 2000.0 / 63
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    assert 148 * nz * nx * 4 > free0
+    rc, h = pdm.pdm_create(nx, nz, nw, 10.0, 10.0, omega, vel, cfg["table"], du, pdm.PDM_PATH_SMEM)
+    assert rc == pdm.PDM_ERR_NOMEM and h is None, rc
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] >= free0 - (64 << 20)          # nothing of the failed plan is left
+    small = pdm_inputs.random_problem(5, 300, 8, 5, 15)
+    assert_parity(pdm, small, pdm.PDM_PATH_SMEM)                       # and the library is still usable
+
+
 def test_delta_table_is_identity_on_gpu(pdm):
     cfg = pdm_inputs.random_problem(3, 520, 9, 4, 25, model="field")
     cfg = dict(cfg, table=pdm_inputs.filters.delta_table(cfg["ntab"], cfg["ntaps"]))
