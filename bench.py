@@ -667,9 +667,12 @@ def measure_3d(args):
     nx = ny = 256; nz = 64; nw = 64
     rows = []
     for ntaps, model, sym in ((7, "layers", False), (7, "field", False), (15, "layers", False), (15, "field", False),
-                              (7, "layers", True), (15, "layers", True), (15, "field", True)):
+                              (7, "layers", True), (15, "layers", True), (15, "field", True), (15, "field", "designed")):
         if True:
-            cfg = pdm_inputs.random_problem_3d(5, nx, ny, nz, nw, ntaps, model=model, symmetric=sym)
+            cfg = pdm_inputs.random_problem_3d(5, nx, ny, nz, nw, ntaps, model=model, symmetric=bool(sym))
+            if sym == "designed":           # 2-D extrapolators from the designed 1-D rows (McClellan transformation)
+                from pdm_inputs import filters
+                cfg["table"] = filters.mcclellan_table(filters.design_table(cfg["ntab"], ntaps, cfg["du"], 1.0))
             P0 = torch.from_numpy(cfg["P0"]).to(dev)
             image = torch.empty((nz, ny, nx), dtype=torch.float32, device=dev)
             with pdm.Plan3D.from_config(cfg, args.flags) as plan:
@@ -690,7 +693,8 @@ def measure_3d(args):
             sps = info["samples"] / t
             hbm_gbs, _ = measured_hbm_gbs()
             rows.append(({"workload": f"3-D nx={nx} ny={ny} nz={nz} nw={nw} taps={ntaps}x{ntaps} velocity={model}"
-                                      + (" operator symmetric in kx, ky (folded kernels)" if sym else ""),
+                                      + (" operator symmetric in kx, ky (folded kernels)" if sym else "")
+                                      + (", McClellan-designed table" if sym == "designed" else ""),
                               "kernel": "pdm3_step", "grid": f"{info['grid_ctas']}x{info['threads_per_cta']}",
                               "smem_bytes": info["smem_bytes"], "steps": args.steps, "ms": t * 1e3,
                               "ms_best": float(min(ms)), "samples_per_s": sps,

@@ -440,6 +440,16 @@ def random_problem(seed: int, nx: int, nz: int, nw: int, ntaps: int, ntab: int =
                 velocity=np.ascontiguousarray(v_in), table=np.ascontiguousarray(table), P0=P0)
 
 
+def diffractor_volume(omega, spectrum, x, y, x0, y0, z0, veff) -> np.ndarray:
+    """Zero-offset (exploding-reflector) record of ONE point diffractor over a 2-D receiver grid:
+    P0(w, y, x) = R(w) exp(-i w t(x, y)) / r,  t = 2 r / veff,  r = sqrt(z0^2 + (x-x0)^2 + (y-y0)^2).
+    complex128 [nw, ny, nx] (the 3-D analogue of diffractor_section)."""
+    r = np.sqrt(z0 * z0 + (np.asarray(x, np.float64)[None, :] - x0) ** 2 + (np.asarray(y, np.float64)[:, None] - y0) ** 2)
+    t = 2.0 * r / veff
+    w = np.asarray(omega, np.float64)
+    return np.asarray(spectrum, np.float64)[:, None, None] * np.exp(-1j * w[:, None, None] * t[None]) / r[None]
+
+
 def random_problem_3d(seed: int, nx: int, ny: int, nz: int, nw: int, ntaps: int, ntab: int = 64,
                       model: str = "field", symmetric: bool = False):
     """Seeded 3-D problem: velocity [nz, ny, nx] ('const' | 'layers' | 'field' = smooth in

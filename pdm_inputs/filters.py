@@ -107,6 +107,49 @@ def design_table(ntab: int, ntaps: int, du: float, r: float = 1.0,
     return np.ascontiguousarray(table)
 
 
+def mcclellan_table(table1d: np.ndarray) -> np.ndarray:
+    """2-D extrapolators for the 3-D variant ("requires 2-D filters as extrapolators"; ref :177)
+    from a symmetric 1-D table by the McClellan transformation: with the 1-D response written as
+        H(kappa) = W_0 + 2 sum_n W_n cos(n kappa) = sum_n a_n T_n(cos kappa),  a_0 = W_0, a_n = 2 W_n,
+    cos kappa is replaced by the 9-point approximation of cos sqrt(kx^2 + ky^2),
+        M(kx, ky) = -1 + (1 + cos kx)(1 + cos ky) / 2
+    (3 x 3 kernel: centre -1/2, edge neighbours 1/4, corners 1/8), and the Chebyshev recurrence
+    T_n = 2 M T_{n-1} - T_{n-2} is run on 2-D kernels (convolutions).  Exact along the axes (M(kx, 0) =
+    cos kx), circularly symmetric to O(k^4) elsewhere.  Returns complex64 [ntab, ntaps, ntaps], symmetric in
+    kx and in ky bit for bit, |H2(kx, ky)| = |H(arccos M)| <= max|H| (stability carries over).
+    Input generator only: both the oracle and the CUDA path receive the table as an array."""
+    t = np.asarray(table1d)
+    ntab, ntaps = t.shape
+    L = (ntaps - 1) // 2
+    a = t[:, L:].astype(np.complex128).copy()
+    a[:, 1:] *= 2.0
+    m = np.array([[0.125, 0.25, 0.125], [0.25, -0.5, 0.25], [0.125, 0.25, 0.125]])
+
+    def conv_m(k):                                   # k: [2L+1, 2L+1] kernel centred at (L, L); support grows by 1
+        out = np.zeros_like(k)
+        for dy in (-1, 0, 1):
+            for dx in (-1, 0, 1):
+                w = m[dy + 1, dx + 1]
+                ys = slice(max(0, dy), ntaps + min(0, dy)); yd = slice(max(0, -dy), ntaps + min(0, -dy))
+                xs = slice(max(0, dx), ntaps + min(0, dx)); xd = slice(max(0, -dx), ntaps + min(0, -dx))
+                out[ys, xs] += w * k[yd, xd]
+        return out
+
+    cheb = [np.zeros((ntaps, ntaps)), None]
+    cheb[0][L, L] = 1.0
+    kernels = [cheb[0]]
+    if L >= 1:
+        kernels.append(conv_m(cheb[0]))
+    for n in range(2, L + 1):
+        kernels.append(2.0 * conv_m(kernels[n - 1]) - kernels[n - 2])
+    basis = np.stack(kernels)                        # [L+1, ntaps, ntaps], real
+    out = np.tensordot(a, basis, axes=(1, 0)).astype(np.complex64)
+    q = out[:, L:, L:]                               # enforce the double mirror symmetry bit for bit
+    out = np.concatenate([np.concatenate([q[:, :0:-1, :0:-1], q[:, :0:-1, :]], 2),
+                          np.concatenate([q[:, :, :0:-1], q], 2)], 1)
+    return np.ascontiguousarray(out)
+
+
 def delta_table(ntab: int, ntaps: int) -> np.ndarray:
     """Identity extrapolator (W_0 = 1, every other tap 0) for every entry: pin P1 input."""
     t = np.zeros((ntab, ntaps), dtype=np.complex64)

@@ -72,6 +72,39 @@ def test_3d_doubly_symmetric_operators_run_folded(pdm, model, nx, ny, nz, nw, nt
     assert rc == (pdm.PDM_ERR_TABLE_ASYMMETRIC if ntaps > 1 else pdm.PDM_OK) and h is None
 
 
+def test_3d_designed_extrapolators_focus_a_diffractor_on_the_device(pdm):
+    """A physically meaningful 3-D run: 15 x 15 extrapolators made from the designed 1-D rows
+    by the McClellan transformation (pdm_inputs/filters.py::mcclellan_table), laterally varying velocity for
+    parity with pdm_oracle_migrate3d, constant velocity for the focusing check of oracle pin T-P6 on the GPU."""
+    import torch
+    from pdm_inputs import filters
+    from pdm_inputs.configs import dft_bin_omegas, ricker_spectrum, diffractor_volume
+    nx, ny, nz, dx, dz, v = 56, 48, 40, 10.0, 10.0, 2000.0
+    omega = dft_bin_omegas(256, 4e-3, 8.0, 45.0)
+    ntab, ntaps = 64, 15
+    x, y = np.arange(nx) * dx, np.arange(ny) * dx
+    x0, y0, z0 = 310.0, 200.0, 250.0
+    P0 = diffractor_volume(omega, ricker_spectrum(omega, 22.0), x, y, x0, y0, z0, v).astype(np.complex64)
+    xs, ys = np.meshgrid(x, y)
+    models = {"const": np.full((nz, ny, nx), 0.5 * v),
+              "field": 0.5 * (v + 400.0 * np.sin(xs / 90.0 + ys / 130.0)[None] + 6.0 * np.arange(nz)[:, None, None])}
+    for name, v_in in models.items():
+        v_in = np.ascontiguousarray(v_in, dtype=np.float32)
+        du = float(omega.max()) * dz / float(v_in.min()) / (ntab - 1)
+        table = filters.mcclellan_table(filters.design_table(ntab, ntaps, du, dz / dx))
+        cfg = dict(nx=nx, ny=ny, nz=nz, nw=omega.size, dz=dz, dx=dx, dy=dx, du=du, omega=omega, velocity=v_in,
+                   table=table, ntab=ntab, ntaps=ntaps, P0=P0)
+        ref = oracle.migrate3d(cfg)
+        with pdm.Plan3D.from_config(cfg) as plan:
+            assert plan.info["table_symmetric"] == 1                   # circularly built: the folded kernels
+            img = plan.migrate(torch.from_numpy(P0).cuda()).cpu().numpy()
+        rel, mx = _errors(img, ref)
+        assert rel <= 1e-4 and mx <= 1e-3, (name, rel, mx)
+        if name == "const":
+            iz, iy, ix = np.unravel_index(np.argmax(np.abs(img)), img.shape)
+            assert abs(ix - round(x0 / dx)) <= 1 and abs(iy - round(y0 / dx)) <= 1 and abs(iz - (round(z0 / dz) - 1)) <= 1
+
+
 def test_3d_force_general_and_unaligned_input(pdm):
     import torch
     cfg = pdm_inputs.random_problem_3d(9, 200, 12, 4, 3, 5, model="layers")

@@ -7,6 +7,9 @@
   T-P4  separable table W[ky][kx] = a[ky] b[kx], constant velocity: the 3-D step is the pinned 1-D
         oracle applied along x with b and along y with a (pdm_oracle_migrate's own wavefields)
   T-P5  transposition: swapping the roles of x and y (inputs, velocity and table) transposes the image
+  T-P6  physics: with 2-D extrapolators made from the designed 1-D rows by the McClellan transformation
+        (pdm_inputs/filters.py::mcclellan_table; PAPER.md:41, ref :177), the zero-offset record of a point
+        diffractor in constant velocity focuses at (x0, y0, z0) +- 1 cell, and conjugated data does not
 """
 import numpy as np
 import pytest
@@ -135,3 +138,42 @@ def test_TP5_transposition():
     imgT = oracle.migrate3d(_cfg3(ny, nx, nz, omega, v.transpose(0, 2, 1), table.transpose(0, 2, 1), du,
                                   P0.transpose(0, 2, 1)))
     np.testing.assert_allclose(imgT, img.transpose(0, 2, 1), rtol=0, atol=1e-13 * np.abs(img).max())
+
+
+def test_TP6_point_diffractor_focuses_in_3d():
+    """Pins what T-P1..T-P5 cannot (they are self-consistent under any sign or axis convention): the sign
+    of the phase (R4), the half velocity (R2), row <-> depth (R6) and the (ky, kx) <-> (y, x) table
+    orientation of R18, through pdm_oracle_migrate3d with a physically meaningful table."""
+    from pdm_inputs import filters
+    from pdm_inputs.configs import dft_bin_omegas, ricker_spectrum, diffractor_volume
+    nx, ny, nz, dx, dz, v = 56, 48, 40, 10.0, 10.0, 2000.0
+    omega = dft_bin_omegas(256, 4e-3, 8.0, 45.0)
+    v_in = 0.5 * v
+    ntab, ntaps = 64, 15
+    du = float(omega.max()) * dz / v_in / (ntab - 1)
+    table = filters.mcclellan_table(filters.design_table(ntab, ntaps, du, dz / dx))
+    L = (ntaps - 1) // 2
+    assert np.array_equal(table[:, ::-1, :].view(np.uint64), table.view(np.uint64))      # symmetric in ky
+    assert np.array_equal(table[:, :, ::-1].view(np.uint64), table.view(np.uint64))      # and in kx
+    # along the kx axis the 2-D response IS the 1-D response (M(kx, 0) = cos kx)
+    row1 = filters.design_table(ntab, ntaps, du, dz / dx)[40].astype(np.complex128)
+    kap = np.linspace(0.0, 2.0, 9)
+    k = np.arange(-L, L + 1)
+    h1 = (row1[None, :] * np.exp(-1j * kap[:, None] * k[None, :])).sum(1)
+    h2 = (table[40].astype(np.complex128).sum(0)[None, :] * np.exp(-1j * kap[:, None] * k[None, :])).sum(1)
+    assert np.abs(h1 - h2).max() < 1e-5
+    x, y = np.arange(nx) * dx, np.arange(ny) * dx
+    x0, y0, z0 = 310.0, 200.0, 250.0                      # deliberately not symmetric in x and y
+    P0 = diffractor_volume(omega, ricker_spectrum(omega, 22.0), x, y, x0, y0, z0, v)
+    cfg = _cfg3(nx, ny, nz, omega, v_in, table, du, P0, dz=dz)
+    img = oracle.migrate3d(cfg)
+    iz, iy, ix = np.unravel_index(np.argmax(np.abs(img)), img.shape)
+    assert abs(ix - round(x0 / dx)) <= 1 and abs(iy - round(y0 / dx)) <= 1, (ix, iy)
+    assert abs(iz - (round(z0 / dz) - 1)) <= 1, iz
+    far = np.abs(img).copy()
+    far[max(0, iz - 6):iz + 7, max(0, iy - 6):iy + 7, max(0, ix - 6):ix + 7] = 0
+    assert far.max() < 0.5 * np.abs(img[iz, iy, ix])
+    bad = oracle.migrate3d(dict(cfg, P0=np.conj(cfg["P0"])))                           # wrong sign convention
+    assert np.abs(bad[iz, iy, ix]) < 0.5 * np.abs(img[iz, iy, ix])
+    worse = oracle.migrate3d(dict(cfg, table=np.conj(table)))                          # conjugated operator
+    assert np.abs(worse[iz, iy, ix]) < 0.5 * np.abs(img[iz, iy, ix])
