@@ -78,7 +78,7 @@ def table_index(omega, velocity, dz: float, du: float, ntab: int) -> int:
                                         float(dz), float(du), int(ntab)))
 
 
-def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field, ntaper=0):
+def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field, ntaper=0, interp=False):
     lib = _load()
     omega = np.ascontiguousarray(omega, dtype=np.float32)
     velocity = np.ascontiguousarray(velocity, dtype=np.float32)
@@ -94,7 +94,16 @@ def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field
         assert nsub > 0 and sub.min() >= 0 and sub.max() < nw
     image = np.zeros((nz, nx), dtype=np.float64)
     field = np.zeros((nlines, nx), dtype=np.complex128) if want_field else None
-    if ntaper:
+    if interp:
+        assert not ntaper
+        lib.pdm_oracle_migrate_interp.restype = ctypes.c_int
+        lib.pdm_oracle_migrate_interp.argtypes = lib.pdm_oracle_migrate.argtypes
+        rc = lib.pdm_oracle_migrate_interp(
+            nx, nz, nw, float(dz), omega.ctypes.data, velocity.ctypes.data,
+            table.ctypes.data, ntab, ntaps, float(du), P0.ctypes.data,
+            None if sub is None else sub.ctypes.data, nsub,
+            image.ctypes.data, None if field is None else field.ctypes.data)
+    elif ntaper:
         rc = lib.pdm_oracle_migrate_taper(
             nx, nz, nw, float(dz), omega.ctypes.data, velocity.ctypes.data,
             table.ctypes.data, ntab, ntaps, float(du), P0.ctypes.data,
@@ -111,11 +120,12 @@ def _run(nx, nz, nw, dz, omega, velocity, table, du, P0, omega_index, want_field
     return image, field
 
 
-def migrate(cfg: dict, omega_index=None, ntaper: int = 0) -> np.ndarray:
+def migrate(cfg: dict, omega_index=None, ntaper: int = 0, interp: bool = False) -> np.ndarray:
     """image float64 [nz, nx] for a workload dict (pdm_inputs layout); optional omega subset;
-    ntaper > 0: the absorbing edge-taper variant of R5 (reading R5b)."""
+    ntaper > 0: the absorbing edge-taper variant of R5 (reading R5b); interp: the operator is the linear
+    blend of the two table rows bracketing u (reading R3c) instead of the nearest row."""
     img, _ = _run(cfg["nx"], cfg["nz"], cfg["nw"], cfg["dz"], cfg["omega"], cfg["velocity"],
-                  cfg["table"], cfg["du"], cfg["P0"], omega_index, False, ntaper)
+                  cfg["table"], cfg["du"], cfg["P0"], omega_index, False, ntaper, interp)
     return img
 
 

@@ -111,12 +111,52 @@ static double oracle_taper(int x, int nx, int ntaper)
     return s * s;
 }
 
+/* R3 variant (reading R3c; SURVEY 8(f) N3 "optional linear interpolation between rows";
+ * PAPER.md:65, :83 only say the filter is looked up): instead of the nearest row, the operator is the
+ * linear blend of the two rows that bracket u = w*dz/v,
+ *     u32 = fl32(w32 * q32)   (the SAME float product as O6),  j0 = floor(u32),  a = u32 - j0  (exact in float),
+ *     W_k = (1 - a) table[j0][k] + a table[j0 + 1][k],         j0 >= ntab-1:  W_k = table[ntab-1][k].
+ * a == 0 wherever u32 is an integer, so the blend then equals the nearest-row operator.           */
+static void oracle_interp_rows(float w32, float q32, int ntab, int *j0, int *j1, double *a)
+{
+    float u = w32 * q32;
+    if (!(u > 0.0f)) u = 0.0f;
+    const float f = floorf(u);
+    if (f >= (float)(ntab - 1)) { *j0 = ntab - 1; *j1 = ntab - 1; *a = 0.0; return; }
+    *j0 = (int)f;
+    *j1 = *j0 + 1;
+    *a = (double)(u - f);
+}
+
+static int oracle_migrate_core(int nx, int nz, int nw, double dz,
+                               const float *omega, const float *velocity,
+                               const oracle_c64 *table, int ntab, int ntaps, double du,
+                               const oracle_c64 *P0,
+                               const int *omega_index, int nsub, int ntaper, int interp,
+                               double *image_out, double *wavefield_out);
+
 int pdm_oracle_migrate_taper(int nx, int nz, int nw, double dz,
                              const float *omega, const float *velocity,
                              const oracle_c64 *table, int ntab, int ntaps, double du,
                              const oracle_c64 *P0,
                              const int *omega_index, int nsub, int ntaper,
-                             double *image_out, double *wavefield_out);
+                             double *image_out, double *wavefield_out)
+{
+    return oracle_migrate_core(nx, nz, nw, dz, omega, velocity, table, ntab, ntaps, du, P0,
+                               omega_index, nsub, ntaper, 0, image_out, wavefield_out);
+}
+
+/* The interpolated-table variant R3c (plain R5 edges). */
+int pdm_oracle_migrate_interp(int nx, int nz, int nw, double dz,
+                              const float *omega, const float *velocity,
+                              const oracle_c64 *table, int ntab, int ntaps, double du,
+                              const oracle_c64 *P0,
+                              const int *omega_index, int nsub,
+                              double *image_out, double *wavefield_out)
+{
+    return oracle_migrate_core(nx, nz, nw, dz, omega, velocity, table, ntab, ntaps, du, P0,
+                               omega_index, nsub, 0, 1, image_out, wavefield_out);
+}
 
 int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
                        const float *omega, const float *velocity,
@@ -129,12 +169,12 @@ int pdm_oracle_migrate(int nx, int nz, int nw, double dz,
                                     omega_index, nsub, 0, image_out, wavefield_out);
 }
 
-int pdm_oracle_migrate_taper(int nx, int nz, int nw, double dz,
-                             const float *omega, const float *velocity,
-                             const oracle_c64 *table, int ntab, int ntaps, double du,
-                             const oracle_c64 *P0,
-                             const int *omega_index, int nsub, int ntaper,
-                             double *image_out, double *wavefield_out)
+static int oracle_migrate_core(int nx, int nz, int nw, double dz,
+                               const float *omega, const float *velocity,
+                               const oracle_c64 *table, int ntab, int ntaps, double du,
+                               const oracle_c64 *P0,
+                               const int *omega_index, int nsub, int ntaper, int interp,
+                               double *image_out, double *wavefield_out)
 {
     if (nx <= 0 || nz <= 0 || nw <= 0 || ntab <= 0 || ntaps < 1 || (ntaps & 1) == 0 || ntaper < 0 ||
         !(du > 0.0) || !omega || !velocity || !table || !P0 || !image_out)
@@ -188,11 +228,23 @@ int pdm_oracle_migrate_taper(int nx, int nz, int nw, double dz,
                     for (int x = 0; x < nx; ++x) {                      /* O5 */
                         const int j = oracle_idx(w32, qrow[x], ntab);   /* O6 */
                         const oracle_c64 *row = table + (size_t)j * ntaps;
+                        const oracle_c64 *row1 = row;                   /* R3c: second row and weight */
+                        double a1 = 0.0;
+                        if (interp) {
+                            int j0, j1;
+                            oracle_interp_rows(w32, qrow[x], ntab, &j0, &j1, &a1);
+                            row = table + (size_t)j0 * ntaps;
+                            row1 = table + (size_t)j1 * ntaps;
+                        }
                         double ar = 0.0, ai = 0.0;
                         for (int k = -L; k <= L; ++k) {                 /* O7 */
                             int xs = x - k;
                             if (xs < 0 || xs >= nx) continue;
                             double wr = (double)row[L + k].re, wi = (double)row[L + k].im;
+                            if (interp) {
+                                wr = (1.0 - a1) * wr + a1 * (double)row1[L + k].re;
+                                wi = (1.0 - a1) * wi + a1 * (double)row1[L + k].im;
+                            }
                             double pr = P[2 * xs], pi = P[2 * xs + 1];
                             ar += wr * pr - wi * pi;
                             ai += wr * pi + wi * pr;
