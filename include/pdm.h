@@ -106,7 +106,16 @@ typedef enum {
                                     /* t(x) = sin^2((pi/2)(d+1)/(n+1)), d = min(x, nx-1-x) < n.  Always   */
                                     /* the PDM_PATH_PACKED form (AUTO or PACKED path bits); not with      */
                                     /* PDM_PRESTACK.  0 = plain R5                                        */
-#define PDM_FLAGS_VALID  0x3FFFFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
+#define PDM_TABLE_INTERP  (1u << 30) /* interpolated look-up (variant R3c of the nearest-row rule R3; the    */
+                                    /* paper only says the filter is looked up): the     */
+                                    /* operator of an output point is the linear blend of the two table    */
+                                    /* rows bracketing u = w*dz/v,  j0 = floor(fl32(w*q32)), a = the        */
+                                    /* fraction,  W_k = (1-a) table[j0][k] + a table[j0+1][k]; at or beyond */
+                                    /* the last row, that row alone.  Runs on the per-depth-step form only  */
+                                    /* (pdm_info.path = PDM_PATH_NAIVE; AUTO or NAIVE path bits), plain     */
+                                    /* poststack (not with PDM_PRESTACK / PDM_TAPER): the accurate-table    */
+                                    /* reference mode, not a fast path                                      */
+#define PDM_FLAGS_VALID  0x7FFFFFFFu /* any other bit set: PDM_ERR_INVALID_ARG                       */
 
 typedef struct {
     int    path;                 /* PDM_PATH_* actually chosen                                      */

@@ -28,6 +28,7 @@ PDM_PATH_AUTO, PDM_PATH_SMEM, PDM_PATH_TILED, PDM_PATH_NAIVE, PDM_PATH_CLUSTER, 
 PDM_TAPS_AUTO, PDM_TAPS_GLOBAL, PDM_TAPS_SLICE, PDM_TAPS_COMPACT = 0 << 4, 1 << 4, 2 << 4, 3 << 4
 PDM_FORCE_GENERAL, PDM_NO_BALANCE, PDM_REQUIRE_SYMMETRIC, PDM_PRESTACK = 1 << 6, 1 << 7, 1 << 20, 1 << 21
 PDM_THREADS_SHIFT, PDM_CTAS_SHIFT, PDM_TAPER_SHIFT = 8, 16, 22
+PDM_TABLE_INTERP = 1 << 30
 
 EXPORTED_SYMBOLS = ("pdm_create", "pdm_migrate", "pdm_migrate_host", "pdm_migrate_shot", "pdm_migrate_static", "pdm_destroy", "pdm_get_info",
                     "pdm_strerror", "pdm_debug_table_index", "pdm_fp32_peak",

@@ -142,6 +142,9 @@ extern "C" int pdm_create(pdm_plan **out, int nx, int nz, int nw, float dx, floa
     if (prestack && path != PDM_PATH_AUTO && path != PDM_PATH_PACKED) return PDM_ERR_INVALID_ARG;
     const int ntaper = (int)((flags >> PDM_TAPER_SHIFT) & 0xFFu);       // R5b: packed form only
     if (ntaper && (prestack || (path != PDM_PATH_AUTO && path != PDM_PATH_PACKED))) return PDM_ERR_INVALID_ARG;
+    // R3c: interpolated look-up -- the per-depth-step form only, plain poststack
+    const bool interp = (flags & PDM_TABLE_INTERP) != 0;
+    if (interp && (prestack || ntaper || (path != PDM_PATH_AUTO && path != PDM_PATH_NAIVE))) return PDM_ERR_INVALID_ARG;
     std::vector<float> omega2;
     if (prestack) {
         if ((double)2 * nw * (double)nx > 2.0e9) return PDM_ERR_UNSUPPORTED;
@@ -612,7 +615,9 @@ static int build_plan(pdm_plan *p, const float *omega, const float *velocity, co
     if (p->prestack || p->ntaper) {
         if (!have_L) return PDM_ERR_UNSUPPORTED;
         p->path = PDM_PATH_PACKED;
-    } else if (want == PDM_PATH_AUTO)
+    } else if (p->flags & PDM_TABLE_INTERP)
+        p->path = PDM_PATH_NAIVE;
+    else if (want == PDM_PATH_AUTO)
         p->path = (auto_cluster || auto_pair) ? PDM_PATH_CLUSTER
                                : (lines_fit ? PDM_PATH_SMEM : (have_L ? PDM_PATH_TILED : PDM_PATH_NAIVE));
     else p->path = (int)want;
@@ -981,8 +986,12 @@ static int migrate_impl(pdm_plan *p, const pdm_c64 *P0_dev, const pdm_c64 *src_d
         }
         for (int z = 0; z < nz; ++z) {
             float2 *dst = p->d_plane[z & 1];
-            pdm_naive_step<<<g1, 128, 0, st>>>(src, dst, p->d_omega, p->d_q + (size_t)z * p->qstride,
-                                                p->d_table, nx, nw, p->ntab, L);
+            if (p->flags & PDM_TABLE_INTERP)
+                pdm_naive_step_interp<<<g1, 128, 0, st>>>(src, dst, p->d_omega, p->d_q + (size_t)z * p->qstride,
+                                                           p->d_table, nx, nw, p->ntab, L);
+            else
+                pdm_naive_step<<<g1, 128, 0, st>>>(src, dst, p->d_omega, p->d_q + (size_t)z * p->qstride,
+                                                    p->d_table, nx, nw, p->ntab, L);
             pdm_naive_image_row<<<g2, 128, 0, st>>>(dst, image_dev + (size_t)z * nx, nx, nw);
             src = dst;
         }

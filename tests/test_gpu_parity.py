@@ -273,6 +273,27 @@ def test_packed_form_many_items_per_cta(pdm, sym, T, n):
     assert np.array_equal(img, again)
 
 
+@pytest.mark.parametrize("model,nx,nz,nw,ntaps,sym", [
+    ("field", 300, 21, 7, 15, True), ("white", 1000, 13, 5, 25, False), ("layers", 129, 9, 3, 51, True),
+    ("const", 64, 5, 2, 61, True),
+])
+def test_interpolated_table_lookup_matches_oracle(pdm, model, nx, nz, nw, ntaps, sym):
+    """PDM_TABLE_INTERP (reading R3c): the operator is the linear blend of the two rows
+    bracketing u; against pdm_oracle_migrate_interp, and visibly different from the nearest-row image."""
+    cfg = pdm_inputs.random_problem(83, nx, nz, nw, ntaps, ntab=64, model=model, symmetric=sym)
+    img, info = gpu_migrate(pdm, cfg, pdm.PDM_TABLE_INTERP, want_info=True)
+    assert info["path"] == pdm.PDM_PATH_NAIVE
+    ref = oracle.migrate(cfg, interp=True)
+    rel, mx = errors(img, ref)
+    assert rel <= REL_L2_BAR and mx <= MAX_PIX_BAR, (rel, mx)
+    if model != "const":
+        assert errors(img, oracle.migrate(cfg))[0] > 10 * REL_L2_BAR
+    args = (cfg["nx"], cfg["nz"], cfg["nw"], cfg["dx"], cfg["dz"], cfg["omega"], cfg["velocity"], cfg["table"], cfg["du"])
+    for bad in (pdm.PDM_PATH_SMEM, pdm.PDM_PATH_PACKED, pdm.PDM_PRESTACK, 9 << pdm.PDM_TAPER_SHIFT):
+        rc, h = pdm.pdm_create(*args, pdm.PDM_TABLE_INTERP | bad)
+        assert rc == pdm.PDM_ERR_INVALID_ARG and h is None
+
+
 def test_packed_path_with_unaligned_p0_pointer(pdm):
     """Even nx but a P0 that is only 8-byte aligned: TMA cannot address it, so the library repacks it
     into its own plane first; same image bit for bit as the direct descriptor on an aligned P0."""
