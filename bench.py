@@ -41,7 +41,7 @@ UNIT = "samples/s"
 # lanes x 2 flop/FMA x 1.965 GHz max SM clock.  The FFMA-chain microbenchmark (pdm_fp32_peak)
 # reads 71-73 TFLOP/s on this pool; both are reported.
 FP32_PEAK_NOMINAL_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r02_traffic.json")
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r03_traffic.json")
 
 
 def csrc_digest() -> str:
@@ -59,7 +59,7 @@ def csrc_digest() -> str:
 
 def ncu_traffic(config: int, path: str, flags: int, world: int):
     """dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the dominant kernel, from the
-    committed `ncu --set full` capture (profiles/r02_traffic.json) -- only when that capture was
+    committed `ncu --set full` capture (profiles/r03_traffic.json) -- only when that capture was
     taken on exactly these kernel sources, this config and this path; else None with the reason."""
     if world != 1 or flags:
         return None, "no capture for multi-rank runs / non-default flags"
@@ -67,7 +67,7 @@ def ncu_traffic(config: int, path: str, flags: int, world: int):
         with open(TRAFFIC_FILE) as f:
             table = json.load(f)
     except (OSError, ValueError):
-        return None, "profiles/r02_traffic.json absent"
+        return None, "profiles/r03_traffic.json absent"
     for e in table.get("captures", []):
         if e.get("config") == config and e.get("path") == path:
             if e.get("csrc_sha1") != csrc_digest():
